@@ -1,0 +1,224 @@
+"""ctypes front end of the fp64 CPU oracle (oracle/amh_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It never imports, links or calls
+anything under paper_2211_03193_b200/ and the CUDA path never imports it.
+
+The arithmetic lives in amh_oracle.c; this file only marshals numpy arrays.  See that file's header
+for the passages of the paper each function follows and DESIGN.md for the readings R1-R22.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "amh_oracle.c")
+_LIB = os.path.join(_HERE, "libamh_oracle.so")
+
+PROP_UNIFORM, PROP_GRID, PROP_GAUSSIAN = 0, 1, 2
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (plain C, -O2, OpenMP over chains)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp",
+                               "-ffp-contract=off", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class Geom(C.Structure):
+    _fields_ = [(k, C.c_double) for k in (
+        "len_n_ca", "len_ca_c", "len_c_n", "ang_n_ca_c", "ang_ca_c_n", "ang_c_n_ca",
+        "omega", "cb_len", "cb_ang", "cb_dih", "eps")] + [("min_sep", C.c_int), ("pad_", C.c_int)]
+
+
+class _Model(C.Structure):
+    _fields_ = [("L", C.c_int), ("nb", C.c_int), ("E", C.c_void_p),
+                ("c0", C.c_double), ("delta", C.c_double), ("g", Geom)]
+
+
+class _RunParams(C.Structure):
+    _fields_ = [("n_sweeps", C.c_longlong), ("sweep_offset", C.c_longlong),
+                ("n_global", C.c_int), ("n_local", C.c_int), ("window", C.c_int), ("global_first", C.c_int),
+                ("t_start", C.c_double), ("t_end", C.c_double), ("ramp_sweeps", C.c_longlong),
+                ("per_chain_T", C.c_void_p),
+                ("prop_mode", C.c_int), ("grid", C.c_int),
+                ("sigma_start", C.c_double), ("sigma_end", C.c_double), ("ramp_sigma", C.c_longlong),
+                ("seed", C.c_ulonglong), ("chain_offset", C.c_longlong),
+                ("only_k", C.c_int), ("trace_steps", C.c_int), ("n_threads", C.c_int), ("pad_", C.c_int)]
+
+
+class _Outputs(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in (
+        "energy", "best_energy", "best_state", "n_accept_local", "n_accept_global",
+        "n_prop_local", "n_prop_global", "sweep_energy", "trace_prop", "trace_dE", "trace_g", "trace_acc")]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.amho_pair.restype = C.c_double
+        _lib.amho_pair.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_double]
+        _lib.amho_energy_cb.restype = C.c_double
+        _lib.amho_energy_local_cb.restype = C.c_double
+        _lib.amho_energy.restype = C.c_double
+        _lib.amho_energy_local.restype = C.c_double
+        _lib.amho_temperature.restype = C.c_double
+        _lib.amho_temperature.argtypes = [C.c_void_p, C.c_longlong, C.c_longlong]
+    return _lib
+
+
+def _p(a):
+    return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+def num_threads() -> int:
+    return int(lib().amho_num_threads())
+
+
+def philox4x32_10(ctr, key) -> np.ndarray:
+    c = np.asarray(ctr, dtype=np.uint32).copy()
+    k = np.asarray(key, dtype=np.uint32).copy()
+    out = np.zeros(4, dtype=np.uint32)
+    lib().amho_philox4x32_10(_p(c), _p(k), _p(out))
+    return out
+
+
+def default_geom(**over) -> Geom:
+    g = Geom()
+    lib().amho_default_geom(C.byref(g))
+    for k, v in over.items():
+        setattr(g, k, v)
+    return g
+
+
+def coords(s, geom: Geom | None = None):
+    """N, CA, C, CB (each fp64 [L][3]) of one torsion vector s (fp32 [2L]) in the canonical frame (R1, R4)."""
+    s = np.ascontiguousarray(s, dtype=np.float32)
+    L = s.shape[0] // 2
+    g = geom or default_geom()
+    out = [np.zeros((L, 3), dtype=np.float64) for _ in range(4)]
+    lib().amho_coords(C.byref(g), C.c_int(L), _p(s), *[_p(a) for a in out])
+    return tuple(out)
+
+
+class Model:
+    """Energy model: table E = -log(p + eps) in fp64 plus the bin geometry (Eq. 3a, R8)."""
+
+    def __init__(self, distogram, edges, geom: Geom | None = None):
+        p = np.ascontiguousarray(distogram, dtype=np.float32)
+        assert p.ndim == 3 and p.shape[0] == p.shape[1]
+        self.L, self.nb = int(p.shape[0]), int(p.shape[2])
+        e = np.asarray(edges, dtype=np.float32).astype(np.float64)
+        assert e.shape[0] == self.nb + 1
+        self.delta = float((e[-1] - e[0]) / self.nb)
+        self.c0 = float(e[0] + 0.5 * self.delta)
+        self.geom = geom or default_geom()
+        self.E = np.empty(p.shape, dtype=np.float64)
+        lib().amho_table(_p(p), C.c_longlong(p.size), C.c_double(self.geom.eps), _p(self.E))
+        self._m = _Model(self.L, self.nb, self.E.ctypes.data, self.c0, self.delta, self.geom)
+
+    @property
+    def n(self):
+        return 2 * self.L
+
+    def pair(self, i: int, j: int, d: float) -> float:
+        row = self.E[i, j]
+        return float(lib().amho_pair(_p(row), self.nb, self.c0, self.delta, float(d)))
+
+    def energy_cb(self, CB) -> float:
+        CB = np.ascontiguousarray(CB, dtype=np.float64)
+        return float(lib().amho_energy_cb(C.byref(self._m), _p(CB)))
+
+    def energy_local_cb(self, CB, k: int, w: int) -> float:
+        CB = np.ascontiguousarray(CB, dtype=np.float64)
+        return float(lib().amho_energy_local_cb(C.byref(self._m), _p(CB), C.c_int(k), C.c_int(w)))
+
+    def energy(self, states, n_threads: int = 0) -> np.ndarray:
+        s = np.ascontiguousarray(states, dtype=np.float32).reshape(-1, self.n)
+        out = np.zeros(s.shape[0], dtype=np.float64)
+        lib().amho_energy_batch(C.byref(self._m), _p(s), C.c_longlong(s.shape[0]), _p(out), C.c_int(n_threads))
+        return out
+
+    def energy_local(self, s, k: int, w: int) -> float:
+        s = np.ascontiguousarray(s, dtype=np.float32)
+        return float(lib().amho_energy_local(C.byref(self._m), _p(s), C.c_int(k), C.c_int(w)))
+
+    # -- Alg. 1 ---------------------------------------------------------------------------------
+    def _params(self, n_sweeps, sweep_offset, n_global, n_local, window, global_first, t_start, t_end,
+                ramp_sweeps, per_chain_T, prop_mode, grid, sigma_start, sigma_end, ramp_sigma, seed,
+                chain_offset, only_k, trace_steps, n_threads):
+        return _RunParams(n_sweeps, sweep_offset, n_global, n_local, window, int(global_first),
+                          t_start, t_end, ramp_sweeps,
+                          None if per_chain_T is None else per_chain_T.ctypes.data,
+                          prop_mode, grid, sigma_start, sigma_end, ramp_sigma, seed, chain_offset,
+                          only_k, trace_steps, n_threads, 0)
+
+    def run(self, states, n_sweeps, *, n_global=1, n_local=10, window=8, global_first=True,
+            t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
+            sigma_start=0.0, sigma_end=0.0, ramp_sigma=0, seed=1, chain_offset=0, sweep_offset=0,
+            only_k=-1, trace_steps=0, n_threads=0, record_sweeps=False):
+        """Free-running AMH; returns a dict (states are returned, the input is not modified)."""
+        s = np.array(states, dtype=np.float32, order="C").reshape(-1, self.n)
+        B = s.shape[0]
+        pct = None if per_chain_T is None else np.ascontiguousarray(per_chain_T, dtype=np.float32)
+        prm = self._params(n_sweeps, sweep_offset, n_global, n_local, window, global_first, t_start, t_end,
+                           ramp_sweeps, pct, prop_mode, grid, sigma_start, sigma_end, ramp_sigma, seed,
+                           chain_offset, only_k, trace_steps, n_threads)
+        r = dict(
+            energy=np.zeros(B), best_energy=np.zeros(B), best_state=np.zeros((B, self.n), np.float32),
+            n_accept_local=np.zeros(B, np.int64), n_accept_global=np.zeros(B, np.int64),
+            n_prop_local=np.zeros(B, np.int64), n_prop_global=np.zeros(B, np.int64),
+            sweep_energy=np.zeros((B, n_sweeps)) if record_sweeps else None,
+            trace_prop=np.zeros((B, trace_steps), np.float32) if trace_steps else None,
+            trace_dE=np.zeros((B, trace_steps)) if trace_steps else None,
+            trace_g=np.zeros((B, trace_steps)) if trace_steps else None,
+            trace_acc=np.zeros((B, trace_steps), np.uint8) if trace_steps else None)
+        o = _Outputs(*[None if r[k] is None else r[k].ctypes.data for k, _ in _Outputs._fields_])
+        rc = lib().amho_run(C.byref(self._m), C.byref(prm), _p(s), C.c_longlong(B), C.byref(o))
+        if rc != 0:
+            raise ValueError("amho_run: invalid argument")
+        r["states"] = s
+        return r
+
+    def follow(self, states, steps, forced_acc, *, n_global=1, n_local=10, window=8, global_first=True,
+               t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
+               sigma_start=0.0, sigma_end=0.0, ramp_sigma=0, seed=1, chain_offset=0, sweep_offset=0,
+               n_threads=0):
+        """Follow mode: replay `steps` proposals taking the decisions in forced_acc [B][steps]."""
+        s = np.array(states, dtype=np.float32, order="C").reshape(-1, self.n)
+        B = s.shape[0]
+        fa = np.ascontiguousarray(forced_acc, dtype=np.uint8).reshape(B, steps)
+        pct = None if per_chain_T is None else np.ascontiguousarray(per_chain_T, dtype=np.float32)
+        prm = self._params(0, sweep_offset, n_global, n_local, window, global_first, t_start, t_end,
+                           ramp_sweeps, pct, prop_mode, grid, sigma_start, sigma_end, ramp_sigma, seed,
+                           chain_offset, -1, 0, n_threads)
+        prop = np.zeros((B, steps), np.float32)
+        dE = np.zeros((B, steps))
+        g = np.zeros((B, steps))
+        acc = np.zeros((B, steps), np.uint8)
+        rc = lib().amho_follow(C.byref(self._m), C.byref(prm), _p(s), C.c_longlong(B), C.c_int(steps),
+                               _p(fa), _p(prop), _p(dE), _p(g), _p(acc))
+        if rc != 0:
+            raise ValueError("amho_follow: invalid argument")
+        return dict(states=s, prop=prop, dE=dE, g=g, acc=acc)
+
+    def temperature(self, t, row=0, **kw) -> float:
+        d = dict(n_sweeps=0, sweep_offset=0, n_global=1, n_local=1, window=0, global_first=True, t_start=1.0,
+                 t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=0, grid=0, sigma_start=0.0,
+                 sigma_end=0.0, ramp_sigma=0, seed=0, chain_offset=0, only_k=-1, trace_steps=0, n_threads=0)
+        d.update(kw)
+        if d["per_chain_T"] is not None:
+            d["per_chain_T"] = np.ascontiguousarray(d["per_chain_T"], dtype=np.float32)
+        prm = self._params(**d)
+        return float(lib().amho_temperature(C.byref(prm), C.c_longlong(t), C.c_longlong(row)))
