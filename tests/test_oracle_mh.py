@@ -1,0 +1,250 @@
+"""Pins P4, P5(iii), P6, P7 and the R5/R7 draw formulas: the oracle's Alternating MH (Alg. 1,
+PAPER.md:97-123; Eq. 1a-1c :27-37; Eq. 2a-2b :43-49) against what the mathematics fixes.
+
+None of the expected values here come from the oracle's own run loop: the Boltzmann laws are
+enumerated state by state, the schedule counts are arithmetic, the draw formulas are retyped in
+numpy from the Philox words.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy import stats
+
+import amh_inputs as gi
+
+
+def _chi2_p(counts, expect):
+    """Pearson chi-square p-value with cells of expectation < 5 merged into one."""
+    counts = np.asarray(counts, float)
+    expect = np.asarray(expect, float)
+    small = expect < 5.0
+    c = np.concatenate([counts[~small], [counts[small].sum()]]) if small.any() else counts
+    e = np.concatenate([expect[~small], [expect[small].sum()]]) if small.any() else expect
+    keep = e > 0
+    c, e = c[keep], e[keep]
+    x2 = float(((c - e) ** 2 / e).sum())
+    return float(stats.chi2.sf(x2, len(e) - 1)), len(e)
+
+
+def _grid_value(m, G):
+    return np.float32((2 * m - G) / np.float32(G)) * np.float32(math.pi)
+
+
+@pytest.mark.parametrize("T", [1.0, 2.5])
+def test_global_mh_samples_the_boltzmann_law_L4(orc, synth, T):
+    # P4 (Eq. 1a-1c): L = 4, min_sep 3 -> one pair (0,3); phi_0 and psi_3 are inert (R1), the other six
+    # torsions on a 4-point grid give 4^6 = 4096 states whose Boltzmann weights are enumerated.
+    # Systematic-scan single-flip MH with a symmetric proposal leaves that law invariant.
+    L, G, n = 4, 4, 8
+    ref, p, edges, m = synth(L, 1000)
+    eff = [1, 2, 3, 4, 5, 6]
+    idx = np.stack(np.meshgrid(*[np.arange(G)] * 6, indexing="ij"), -1).reshape(-1, 6)
+    states = np.zeros((len(idx), n), np.float32)
+    states[:, 0] = _grid_value(1, G); states[:, 7] = _grid_value(2, G)
+    for q, v in enumerate(eff):
+        states[:, v] = _grid_value(idx[:, q], G)
+    V = m.energy(states)
+    assert V.max() - V.min() > 1.0            # the law is far from uniform, so the test has power
+    w = np.exp(-(V - V.min()) / T)
+    prob = w / w.sum()
+
+    B = 65536
+    start = gi.grid_states(B, n, G, seed=11)
+    r = m.run(start, 40, n_global=1, n_local=0, window=0, t_start=T, t_end=T,
+              prop_mode=orc.PROP_GRID, grid=G, seed=5)
+    s = r["states"]
+    cell = np.zeros(B, np.int64)
+    for v in eff:
+        mm = np.rint((s[:, v].astype(np.float64) / math.pi * G + G) / 2).astype(np.int64)
+        assert np.all((mm >= 0) & (mm < G))
+        cell = cell * G + mm
+    counts = np.bincount(cell, minlength=G ** 6)
+    pval, cells = _chi2_p(counts, B * prob)
+    assert cells > 500
+    assert pval > 0.01, pval
+    # the inert variables are always accepted, hence uniform on the grid
+    for v in (0, 7):
+        mm = np.rint((s[:, v].astype(np.float64) / math.pi * G + G) / 2).astype(np.int64)
+        pv, _ = _chi2_p(np.bincount(mm, minlength=G), np.full(G, B / G))
+        assert pv > 0.001
+    # a wrong acceptance (inverted ratio) would instead concentrate on HIGH energies: check the mean
+    assert abs(float(V[cell].mean()) - float((prob * V).sum())) < 0.05
+
+
+def test_global_mh_boltzmann_L3_three_pairs(orc):
+    # P4, second case: L = 3 with min_sep = 1 -> three pairs; effective torsions psi_0, phi_1, psi_1, phi_2
+    L, G, n = 3, 6, 6
+    g = orc.default_geom(min_sep=1)
+    ref = gi.reference_torsions(L, 77)
+    CB = orc.coords(ref, g)[3]
+    D = np.linalg.norm(CB[:, None] - CB[None], axis=-1)
+    # C-beta distances at L = 3 only span ~3.5-7.5 A: use a narrow bin range so several bins matter
+    p = gi.distogram_from_distances(D, n_bins=16, lo=3.0, hi=8.0, sigma=0.5)
+    m = orc.Model(p, gi.bin_edges(16, 3.0, 8.0), g)
+    eff = [1, 2, 3, 4]
+    idx = np.stack(np.meshgrid(*[np.arange(G)] * 4, indexing="ij"), -1).reshape(-1, 4)
+    states = np.zeros((len(idx), n), np.float32)
+    for q, v in enumerate(eff):
+        states[:, v] = _grid_value(idx[:, q], G)
+    V = m.energy(states)
+    assert V.max() - V.min() > 2.0
+    prob = np.exp(-(V - V.min())); prob /= prob.sum()
+    B = 40000
+    r = m.run(gi.grid_states(B, n, G, seed=3), 30, n_global=1, n_local=0, window=0,
+              prop_mode=orc.PROP_GRID, grid=G, seed=9)
+    cell = np.zeros(B, np.int64)
+    for v in eff:
+        cell = cell * G + np.rint((r["states"][:, v].astype(np.float64) / math.pi * G + G) / 2).astype(np.int64)
+    pval, cells = _chi2_p(np.bincount(cell, minlength=G ** 4), B * prob)
+    assert cells > 100 and pval > 0.01, (cells, pval)
+
+
+@pytest.mark.parametrize("k", [9, 14])
+def test_fixed_k_local_chain_samples_exp_minus_Vlocal(orc, synth, k):
+    # P5 (iii) (Eq. 2a-2b, 3b): proposing only variable k, the chain on s_k is plain MH for
+    # exp(-V_local(G(s), k, w) / T) over the G grid values of s_k - enumerable.  All chains start from
+    # the same state, so the burn-in (150 proposals of s_k) has to cover the slowest mode.
+    L, w, G, T = 16, 3, 8, 3.0
+    ref, p, edges, m = synth(L, 1000)
+    base = gi.grid_states(1, 2 * L, G, seed=21)[0]
+    cand = np.repeat(base[None], G, 0)
+    cand[:, k] = _grid_value(np.arange(G), G)
+    Vl = np.array([m.energy_local(c, k, w) for c in cand])
+    assert Vl.max() - Vl.min() > 0.5
+    prob = np.exp(-(Vl - Vl.min()) / T); prob /= prob.sum()
+    B = 30000
+    r = m.run(np.repeat(base[None], B, 0), 150, n_global=0, n_local=1, window=w, t_start=T, t_end=T,
+              prop_mode=orc.PROP_GRID, grid=G, seed=4, only_k=k)
+    s = r["states"]
+    other = np.delete(np.arange(2 * L), k)
+    assert np.array_equal(s[:, other], np.repeat(base[None, other], B, 0))     # nothing else moved
+    mm = np.rint((s[:, k].astype(np.float64) / math.pi * G + G) / 2).astype(np.int64)
+    pval, _ = _chi2_p(np.bincount(mm, minlength=G), B * prob)
+    assert pval > 0.01, pval
+    # and it is NOT the law of the global energy (the window matters)
+    Vg = m.energy(cand)
+    pg = np.exp(-(Vg - Vg.min()) / T); pg /= pg.sum()
+    assert np.abs(pg - prob).max() > 0.02
+
+
+def test_draw_formulas_R5_R7(orc, synth):
+    # R5 (UNIFORM proposal) and R7 (u in (0,1]) retyped from the Philox words; R6 keying.
+    # With w = 0 the window holds one residue, so every local dE is exactly 0 and g = log u.
+    L, B, steps = 6, 3, 24
+    ref, p, edges, m = synth(L, 1000)
+    s0 = gi.initial_states(B, 2 * L, 2)
+    seed = (0xDEADBEEF << 32) | 0x12345678
+    r = m.run(s0, 2, n_global=0, n_local=1, window=0, seed=seed, chain_offset=5, trace_steps=steps)
+    for b in range(B):
+        for q in range(steps):
+            key = [seed & 0xFFFFFFFF, seed >> 32]
+            xp = orc.philox4x32_10([q, 0, 5 + b, 0], key)
+            xa = orc.philox4x32_10([q, 0, 5 + b, 1], key)
+            h = np.int64(xp[0] >> 8) - (1 << 23)
+            want = np.float32(np.float32(h) * np.float32(2.0 ** -23)) * np.float32(math.pi)
+            assert r["trace_prop"][b, q] == want
+            u = (float(xa[0] >> 8) + 1.0) * 2.0 ** -24
+            assert 0.0 < u <= 1.0
+            assert r["trace_dE"][b, q] == 0.0
+            assert r["trace_g"][b, q] == pytest.approx(math.log(u), abs=1e-15)
+            assert r["trace_acc"][b, q] == 1
+    assert np.array_equal(r["states"], r["trace_prop"][:, 12:24])    # all accepted: last sweep's proposals
+    # the proposal value covers [-pi, pi) and never reaches +pi
+    assert -math.pi <= float(r["trace_prop"].min()) and float(r["trace_prop"].max()) < math.pi
+
+
+def test_schedule_counts_and_phase_order(orc, synth):
+    # P6 / R10: cycle = n_global global sweeps then n_local local sweeps; n_sweeps counts all sweeps.
+    # cfg 0 shape: the first 1000 steps are 128 global + 872 local proposals (R21).  With w = 0 every
+    # local dE is exactly 0, so the trace shows which steps were judged on the global energy.
+    c0 = gi.CONFIGS[0]
+    ref, p, edges, m = synth(c0.L, c0.cfg_seed)
+    s0 = gi.initial_states(2, c0.n, 1)
+    r = m.run(s0, 22, n_global=c0.n_global, n_local=c0.n_local, window=0, seed=1, trace_steps=1000)
+    assert np.all(r["n_prop_global"] == 2 * c0.n) and np.all(r["n_prop_local"] == 20 * c0.n)
+    nz = r["trace_dE"] != 0.0
+    assert np.all(nz[:, 1:127])             # global sweep: every variable but the two inert ones moves CB
+    assert not nz[:, 0].any() and not nz[:, 127].any()      # phi_0, psi_{L-1} inert (R1)
+    assert not nz[:, 128:].any()            # steps 128..999 are local
+    # local-first ordering
+    r2 = m.run(s0, 3, n_global=1, n_local=2, window=0, global_first=False, seed=1, trace_steps=3 * c0.n)
+    nz2 = (r2["trace_dE"] != 0.0).reshape(2, 3, c0.n).any(axis=2)
+    assert np.array_equal(nz2, np.array([[False, False, True]] * 2))
+    # sweep_offset continues the cycle where it left off
+    r3 = m.run(s0, 2, n_global=1, n_local=2, window=0, seed=1, sweep_offset=2, trace_steps=2 * c0.n)
+    nz3 = (r3["trace_dE"] != 0.0).reshape(2, 2, c0.n).any(axis=2)
+    assert np.array_equal(nz3, np.array([[False, True]] * 2))
+    assert c0.proposals == 32 * 2200 * 128
+
+
+def test_temperature_schedule(orc, synth):
+    # P6 / R13: geometric per sweep with exact endpoints; per-chain constants override the ramp
+    ref, p, edges, m = synth(8, 1000)
+    S = 20001
+    kw = dict(t_start=10.0, t_end=0.1, ramp_sweeps=S)
+    assert m.temperature(0, **kw) == 10.0
+    assert m.temperature(S - 1, **kw) == 0.1
+    assert m.temperature(S + 50, **kw) == 0.1
+    assert m.temperature((S - 1) // 2, **kw) == pytest.approx(1.0, rel=1e-13)
+    assert m.temperature(5000, **kw) == pytest.approx(10.0 * 0.01 ** 0.25, rel=1e-13)
+    assert m.temperature(7, t_start=1.0, t_end=1.0, ramp_sweeps=0) == 1.0
+    pct = gi.per_chain_temperature(16, 8, 0.1, 5.0)
+    assert pct[0] == np.float32(0.1) and pct[7] == np.float32(5.0) and pct[8] == pct[0]
+    assert np.allclose(pct[1:8] / pct[0:7], 50.0 ** (1 / 7), rtol=1e-6)
+    assert m.temperature(3, row=5, per_chain_T=pct, **kw) == float(pct[5])
+    # a hot chain accepts more than a cold one
+    L = 8
+    s0 = np.repeat(gi.initial_states(1, 2 * L, 3), 64, 0)
+    T = np.where(np.arange(64) < 32, 0.05, 50.0).astype(np.float32)
+    r = m.run(s0, 20, n_global=1, n_local=0, window=0, per_chain_T=T, seed=2)
+    assert r["n_accept_global"][32:].mean() > 1.5 * r["n_accept_global"][:32].mean()
+
+
+def test_determinism_split_runs_and_chain_ids(orc, synth):
+    # P7: counter-based RNG -> same seed, same trajectory; run(a) then run(b, offset=a) == run(a+b);
+    # a row's trajectory depends on its chain id, not on its row index
+    L = 12
+    ref, p, edges, m = synth(L, 1000)
+    s0 = gi.initial_states(6, 2 * L, 4)
+    kw = dict(n_global=1, n_local=2, window=3, seed=17)
+    a = m.run(s0, 9, **kw)
+    b = m.run(s0, 9, **kw)
+    assert np.array_equal(a["states"], b["states"]) and np.array_equal(a["energy"], b["energy"])
+    h1 = m.run(s0, 4, **kw)
+    h2 = m.run(h1["states"], 5, sweep_offset=4, **kw)
+    assert np.array_equal(h2["states"], a["states"])
+    assert np.array_equal(h2["energy"], a["energy"])
+    assert np.all(np.minimum(h1["best_energy"], h2["best_energy"]) == a["best_energy"])
+    assert np.array_equal(h1["n_accept_local"] + h2["n_accept_local"], a["n_accept_local"])
+    assert np.array_equal(h1["n_accept_global"] + h2["n_accept_global"], a["n_accept_global"])
+    c = m.run(s0[3:], 9, chain_offset=3, **kw)
+    assert np.array_equal(c["states"], a["states"][3:])
+    d = m.run(s0, 9, **dict(kw, seed=18))
+    assert not np.array_equal(d["states"], a["states"])
+    # energies reported are the energies of the returned states; best <= every sweep end
+    assert np.allclose(a["energy"], m.energy(a["states"]), rtol=0, atol=1e-9)
+    e = m.run(s0, 9, record_sweeps=True, **kw)
+    assert np.array_equal(e["sweep_energy"].min(axis=1), e["best_energy"])
+    assert np.allclose(m.energy(e["best_state"]), e["best_energy"], rtol=0, atol=1e-9)
+
+
+def test_follow_mode_reproduces_the_free_run(orc, synth):
+    # the parity protocol's replay: forcing the run's own decisions reproduces its trace
+    L, steps = 10, 90
+    ref, p, edges, m = synth(L, 1000)
+    s0 = gi.initial_states(4, 2 * L, 6)
+    kw = dict(n_global=1, n_local=3, window=2, seed=23, t_start=0.7, t_end=0.7)
+    r = m.run(s0, 5, trace_steps=steps, **kw)
+    f = m.follow(s0, steps, r["trace_acc"], **kw)
+    assert np.array_equal(f["prop"], r["trace_prop"])
+    assert np.array_equal(f["dE"], r["trace_dE"])
+    assert np.array_equal(f["acc"], r["trace_acc"])
+    assert np.array_equal(f["g"], r["trace_g"])
+    # accept rule R14: accepted iff g = log u + dE/T <= 0
+    assert np.array_equal(r["trace_acc"].astype(bool), r["trace_g"] <= 0.0)
+    # forcing the opposite decision at one step changes the path from there on
+    forced = r["trace_acc"].copy(); forced[:, 30] ^= 1
+    f2 = m.follow(s0, steps, forced, **kw)
+    assert np.array_equal(f2["dE"][:, :31], r["trace_dE"][:, :31])
+    assert not np.array_equal(f2["states"], f["states"])
