@@ -1,0 +1,182 @@
+/*
+ * amh.h - C ABI of the B200-native Alternating Metropolis-Hastings (AMH) hot path.
+ *
+ * Method: Ghantasala, Jaiswal, Datta, "An Efficient MCMC Approach to Energy Function Optimization in
+ * Protein Structure Prediction", arXiv 2211.03193.  "PAPER.md:<line>" cites the text of that paper,
+ * "Rn" a reading listed in DESIGN.md (taken where the paper is silent, ambiguous or garbled).
+ *
+ * What the library computes (one GPU, hand-written CUDA for sm_100a, no CPU fallback):
+ *   state        s in R^n, n = 2L, s[2i] = phi_i, s[2i+1] = psi_i, radians        PAPER.md:25, Fig. 2 (:67); R15, R16
+ *   geometry     x = G(s): backbone by NeRF with ideal geometry, C-beta from N/CA/C   PAPER.md:39, 77; R1-R4
+ *   energy       V(x) = sum_{i<j, j-i>=min_sep} e_ij(|CB_i - CB_j|)   (Eq. 3a)      PAPER.md:75; R8, R9
+ *                e_ij(d): -log(p_ij + eps) interpolated linearly between bin centres, clamped at the ends
+ *   local energy V_local(x,k,w): the same sum restricted to residues floor(k/2)-w .. floor(k/2)+w
+ *                (Eq. 3b)                                                          PAPER.md:81-86; R12
+ *   MH           single-flip proposal of s_k, accept iff log u <= -dE/T   (Eq. 1a-1c, 2a-2b)
+ *                                                                                  PAPER.md:27-49; R5, R7, R14
+ *   alternation  cycles of n_global sweeps judged on V, then n_local sweeps judged on V_local;
+ *                one sweep = k = 0..n-1 in order   (Alg. 1, Fig. 1)                 PAPER.md:55, 97-123, 129; R10
+ *   RNG          Philox4x32-10, key = seed, counter = (step_lo, step_hi, chain, purpose), step = t*n + k   R6
+ *
+ * Conventions
+ *   - "device" pointers are CUDA device memory of the current device; "host" pointers are ordinary
+ *     host memory.  Each argument says which.  The caller owns every buffer it passes in.
+ *   - All device work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy
+ *     default stream).  amh_run / amh_energy / amh_energy_local / amh_coords do not synchronise and
+ *     do not allocate; the *_host variants and amh_create / amh_destroy synchronise.
+ *   - Every function returns an amh_status; nothing throws or exits.  amh_last_error() returns a
+ *     thread-local, NUL-terminated description of the last failure on this thread.
+ *   - Chain ids: row b of a state batch is chain (chain_offset + b); the id, not the row, keys the RNG,
+ *     so a batch may be sharded across calls or GPUs without changing any trajectory.
+ */
+#ifndef AMH_H_
+#define AMH_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct amh_ctx amh_ctx;   /* opaque; owns the device energy table and the geometry constants */
+
+typedef enum {
+    AMH_OK = 0,
+    AMH_ERR_INVALID_ARG = 1,   /* NULL where a pointer is required, sizes < 1, T <= 0, NaN/Inf/negative p, ... */
+    AMH_ERR_UNSUPPORTED = 2,   /* non-uniform bins, AMH_PARAM_TR5, L beyond the shared-memory plan, Gaussian proposals */
+    AMH_ERR_CUDA = 3,          /* a CUDA runtime call failed; see amh_last_error() */
+    AMH_ERR_OOM = 4
+} amh_status;
+
+typedef enum {
+    AMH_PARAM_PHI_PSI = 0,     /* 2 variables per residue (the paper's AlphaFold1 mapping) */
+    AMH_PARAM_TR5 = 1          /* 5 variables per residue (trRosetta2): not built, AMH_ERR_UNSUPPORTED */
+} amh_param;
+
+/* Geometry and energy options.  amh_default_options() fills the values every config of
+ * BASELINE.json uses (R2, R3, R9).  Lengths in Angstrom, angles in radians. */
+typedef struct {
+    double len_n_ca, len_ca_c, len_c_n;          /* 1.458, 1.525, 1.329 */
+    double ang_n_ca_c, ang_ca_c_n, ang_c_n_ca;   /* 111.2, 116.2, 121.7 degrees */
+    double omega;                                /* pi (trans) */
+    double cb_len, cb_ang, cb_dih;               /* |CA-CB| 1.522, angle N-CA-CB 1.927, dihedral C-N-CA-CB -2.143 */
+    double eps;                                  /* 1e-8, added to p inside the log */
+    int    min_sep;                              /* 3: pairs need j - i >= min_sep; >= 1 */
+    int    warps_per_chain;                      /* amh_run launch shape: 0 = choose from L and B; else 1,2,4,8,16 */
+} amh_options;
+
+/* Alg. 1 / Fig. 1, R10, R12. */
+typedef struct {
+    int n_global;       /* sweeps per cycle judged on V            (>= 0) */
+    int n_local;        /* sweeps per cycle judged on V_local      (>= 0; n_global + n_local >= 1) */
+    int window;         /* radius w in residues, inclusive, clamped at the chain ends (>= 0) */
+    int global_first;   /* 1 = Alg. 1 order (global sweeps first in each cycle); 0 = local first */
+} amh_schedule;
+
+/* R13.  T_t = t_start * (t_end/t_start)^(t/(ramp_sweeps-1)) for absolute sweep index t, constant
+ * within a sweep, clamped to t_end for t >= ramp_sweeps-1; t_start == t_end or ramp_sweeps <= 1 means
+ * constant t_start.  per_chain_T (DEVICE float[B], or NULL) overrides the ramp with one constant
+ * temperature per row (config 4's replicas).  All temperatures must be > 0. */
+typedef struct {
+    double t_start, t_end;
+    long long ramp_sweeps;
+    const float *per_chain_T;
+} amh_temperature;
+
+typedef enum {
+    AMH_PROP_UNIFORM = 0,   /* s'_k = fp32(h * 2^-23) * fp32(pi), h = (x0 >> 8) - 2^23    (BASELINE.json configs; R5) */
+    AMH_PROP_GRID = 1       /* s'_k = fp32((2m - G)/G) * fp32(pi), m = x0 mod G           (tests: Boltzmann pins P4/P5) */
+    /* the paper's Gaussian single flip is DESIGN.md NEXT-1: AMH_ERR_UNSUPPORTED */
+} amh_prop_mode;
+
+typedef struct { int mode; int grid; } amh_proposal;
+
+/* Results of amh_run.  Every pointer is optional (NULL = not wanted).  DEVICE memory for amh_run,
+ * HOST memory for amh_run_host.  B = rows of the batch, n = 2L. */
+typedef struct {
+    float *energy;                        /* [B] V of the final state */
+    float *best_energy;                   /* [B] min over this call's sweep ends of V */
+    float *best_state;                    /* [B][n] the state at that sweep end */
+    unsigned long long *n_accept_local;   /* [B] accepted proposals in local sweeps */
+    unsigned long long *n_accept_global;  /* [B] accepted proposals in global sweeps */
+    long long *first_hit_sweep;           /* [1] smallest absolute sweep index at whose end some chain of the
+                                                 batch had V <= energy_threshold; -1 if none */
+    float energy_threshold;
+    int   trace_steps;                    /* the first trace_steps proposals of the call are traced per chain */
+    float *trace_prop;                    /* [B][trace_steps] proposed value s'_k */
+    double *trace_dE;                     /* [B][trace_steps] dE the decision used */
+    unsigned char *trace_acc;             /* [B][trace_steps] 1 = accepted */
+} amh_outputs;
+
+/* Fill *opt with the defaults above.  opt: host. */
+amh_status amh_default_options(amh_options *opt);
+
+/* Build a context: validate, compute E = -log(p + eps) (Eq. 3a) into device memory.
+ *   out         host; receives the context
+ *   n_res       L >= 1 (L < min_sep + 1 is valid: no pairs, energy 0)
+ *   param       AMH_PARAM_PHI_PSI
+ *   distogram   HOST or DEVICE float [L][L][n_bins] row-major, p_ij(b) >= 0 finite; only i < j is read.
+ *               Copied: the caller may free it after the call.
+ *   bin_edges   HOST float [n_bins + 1], increasing, evenly spaced to 1e-5 relative (else UNSUPPORTED)
+ *   n_bins      >= 2
+ *   opt         host, or NULL for the defaults
+ * Synchronises the stream. */
+amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *distogram,
+                      const float *bin_edges, int n_bins, const amh_options *opt, void *cuda_stream);
+
+/* Free the context and everything it owns (synchronises the device). NULL is allowed. */
+amh_status amh_destroy(amh_ctx *ctx);
+
+/* V(G(s)) for a batch (Eq. 3a).  states: DEVICE float [B][n]; energy_out: DEVICE float [B]. B >= 0. */
+amh_status amh_energy(amh_ctx *ctx, const float *states, long long B, float *energy_out, void *cuda_stream);
+
+/* V_local(G(s), k, window) for a batch (Eq. 3b, R12).  0 <= k < n, window >= 0.  Same layouts. */
+amh_status amh_energy_local(amh_ctx *ctx, const float *states, long long B, int k, int window,
+                            float *energy_out, void *cuda_stream);
+
+/* x = G(s) in the canonical frame (R1, R4: N_0 at the origin, CA_0 on +x, C_0 in the xy plane, y > 0).
+ *   cb_out     DEVICE float  [B][L][3] C-beta, or NULL
+ *   atoms_out  DEVICE double [B][L][4][3] N, CA, C, CB, or NULL */
+amh_status amh_coords(amh_ctx *ctx, const float *states, long long B, float *cb_out, double *atoms_out,
+                      void *cuda_stream);
+
+/* Alg. 1 on a batch of independent chains.
+ *   states        DEVICE float [B][n], in/out
+ *   n_sweeps      sweeps of this call (>= 0), all kinds counted (R10)
+ *   sweep_offset  absolute index of the first sweep (>= 0): it positions the call in the cycle, in the
+ *                 temperature ramp and in the RNG counter, so run(a) then run(b, offset a) == run(a+b)
+ *   chain_offset  chain id of row 0
+ *   sched, temp   host, required
+ *   prop          host, or NULL for AMH_PROP_UNIFORM
+ *   out           host struct of DEVICE pointers, or NULL */
+amh_status amh_run(amh_ctx *ctx, float *states, long long B, long long n_sweeps, long long sweep_offset,
+                   long long chain_offset, const amh_schedule *sched, const amh_temperature *temp,
+                   const amh_proposal *prop, unsigned long long seed, const amh_outputs *out,
+                   void *cuda_stream);
+
+/* The same call on HOST buffers: states, temp->per_chain_T and every pointer in *out are host memory.
+ * Copies in, runs, copies out and synchronises the stream; device staging buffers are owned by the
+ * context and grow on demand. */
+amh_status amh_run_host(amh_ctx *ctx, float *states, long long B, long long n_sweeps, long long sweep_offset,
+                        long long chain_offset, const amh_schedule *sched, const amh_temperature *temp,
+                        const amh_proposal *prop, unsigned long long seed, const amh_outputs *out,
+                        void *cuda_stream);
+
+/* HOST-buffer energy: states host float [B][n] -> energy_out host float [B]; synchronises. */
+amh_status amh_energy_host(amh_ctx *ctx, const float *states, long long B, float *energy_out, void *cuda_stream);
+
+/* Launch shape amh_run would use for a batch of B rows: threads per chain-CTA, dynamic shared memory
+ * bytes per CTA, CTAs resident per SM, SM count.  Any pointer may be NULL.  Host. */
+amh_status amh_launch_info(amh_ctx *ctx, long long B, int *threads_per_chain, int *smem_bytes,
+                           int *ctas_per_sm, int *n_sm);
+
+/* Test hook (pin P0 on the device): out[q][0..3] = Philox4x32-10(ctr[q][0..3], key[q][0..1]).
+ * ctr: DEVICE uint32 [count][4]; key: DEVICE uint32 [count][2]; out: DEVICE uint32 [count][4]. */
+amh_status amh_philox_test(const unsigned int *ctr, const unsigned int *key, unsigned int *out,
+                           long long count, void *cuda_stream);
+
+const char *amh_last_error(void);
+const char *amh_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AMH_H_ */

@@ -1,0 +1,302 @@
+"""paper_2211_03193_b200 - thin Python binding of the AMH C-ABI library (include/amh.h).
+
+Argument marshalling only: every step of the hot path (Philox draws, NeRF geometry, pair energies,
+Metropolis test, book-keeping) runs in the CUDA kernels of csrc/.  PyTorch supplies device memory
+and streams.  There is no CPU fallback: without the compiled library (python -m
+paper_2211_03193_b200.build) or without a CUDA device every call raises.
+
+Names follow include/amh.h: amh_create -> AMH(...), amh_run -> AMH.run, amh_energy -> AMH.energy,
+amh_energy_local -> AMH.energy_local, amh_coords -> AMH.coords, amh_run_host -> AMH.run_host.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+__all__ = ["AMH", "AMHError", "Options", "lib", "lib_path", "default_options", "philox4x32_10",
+           "PROP_UNIFORM", "PROP_GRID", "EXPORTS"]
+
+PROP_UNIFORM, PROP_GRID = 0, 1
+
+# every symbol include/amh.h declares
+EXPORTS = ["amh_default_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
+           "amh_run", "amh_run_host", "amh_energy_host", "amh_launch_info", "amh_philox_test",
+           "amh_last_error", "amh_version"]
+
+
+class AMHError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__("amh status %d: %s" % (status, msg))
+        self.status = status
+
+
+class Options(C.Structure):
+    _fields_ = [(k, C.c_double) for k in (
+        "len_n_ca", "len_ca_c", "len_c_n", "ang_n_ca_c", "ang_ca_c_n", "ang_c_n_ca", "omega",
+        "cb_len", "cb_ang", "cb_dih", "eps")] + [("min_sep", C.c_int), ("warps_per_chain", C.c_int)]
+
+
+class _Schedule(C.Structure):
+    _fields_ = [("n_global", C.c_int), ("n_local", C.c_int), ("window", C.c_int), ("global_first", C.c_int)]
+
+
+class _Temperature(C.Structure):
+    _fields_ = [("t_start", C.c_double), ("t_end", C.c_double), ("ramp_sweeps", C.c_longlong),
+                ("per_chain_T", C.c_void_p)]
+
+
+class _Proposal(C.Structure):
+    _fields_ = [("mode", C.c_int), ("grid", C.c_int)]
+
+
+class _Outputs(C.Structure):
+    _fields_ = [("energy", C.c_void_p), ("best_energy", C.c_void_p), ("best_state", C.c_void_p),
+                ("n_accept_local", C.c_void_p), ("n_accept_global", C.c_void_p),
+                ("first_hit_sweep", C.c_void_p), ("energy_threshold", C.c_float), ("trace_steps", C.c_int),
+                ("trace_prop", C.c_void_p), ("trace_dE", C.c_void_p), ("trace_acc", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Load csrc/libamh_b200.so (fails loudly when it has not been built)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_build.LIB):
+            raise ImportError("%s is missing: run `python -m paper_2211_03193_b200.build` (nvcc, sm_100a); "
+                              "there is no CPU fallback" % _build.LIB)
+        L = C.CDLL(_build.LIB)
+        L.amh_last_error.restype = C.c_char_p
+        L.amh_version.restype = C.c_char_p
+        L.amh_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int,
+                                 C.c_void_p, C.c_void_p]
+        L.amh_destroy.argtypes = [C.c_void_p]
+        L.amh_energy.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p]
+        L.amh_energy_host.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p]
+        L.amh_energy_local.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.amh_coords.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p, C.c_void_p]
+        run_args = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_longlong, C.c_longlong, C.c_longlong,
+                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_ulonglong, C.c_void_p, C.c_void_p]
+        L.amh_run.argtypes = run_args
+        L.amh_run_host.argtypes = run_args
+        L.amh_launch_info.argtypes = [C.c_void_p, C.c_longlong] + [C.POINTER(C.c_int)] * 4
+        L.amh_philox_test.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]
+        L.amh_default_options.argtypes = [C.POINTER(Options)]
+        _lib = L
+    return _lib
+
+
+def _check(st: int):
+    if st != 0:
+        raise AMHError(st, lib().amh_last_error().decode())
+
+
+def default_options(**over) -> Options:
+    o = Options()
+    _check(lib().amh_default_options(C.byref(o)))
+    for k, v in over.items():
+        setattr(o, k, v)
+    return o
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2211_03193_b200 needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+def _stream_ptr(stream=None) -> int:
+    torch = _torch()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _dev(t, dtype, name):
+    torch = _torch()
+    if not isinstance(t, torch.Tensor):
+        t = torch.as_tensor(np.ascontiguousarray(t), device="cuda")
+    if t.dtype != dtype or not t.is_cuda or not t.is_contiguous():
+        t = t.to(device="cuda", dtype=dtype).contiguous()
+    return t
+
+
+def philox4x32_10(ctr, key):
+    """Device Philox4x32-10 of the sweep kernel on arrays ctr [N][4], key [N][2] (test hook)."""
+    torch = _torch()
+    c = torch.as_tensor(np.ascontiguousarray(ctr, dtype=np.uint32).view(np.int32), device="cuda")
+    k = torch.as_tensor(np.ascontiguousarray(key, dtype=np.uint32).view(np.int32), device="cuda")
+    out = torch.empty_like(c)
+    _check(lib().amh_philox_test(c.data_ptr(), k.data_ptr(), out.data_ptr(), c.shape[0], _stream_ptr()))
+    return out.cpu().numpy().view(np.uint32)
+
+
+class AMH:
+    """amh_ctx: energy table on the device + geometry constants (amh_create / amh_destroy)."""
+
+    def __init__(self, distogram, bin_edges, options: Options | None = None, stream=None):
+        torch = _torch()
+        self._h = C.c_void_p()
+        if isinstance(distogram, torch.Tensor):
+            d = distogram.to(dtype=torch.float32).contiguous()
+            dptr, shape = d.data_ptr(), tuple(d.shape)
+        else:
+            d = np.ascontiguousarray(distogram, dtype=np.float32)
+            dptr, shape = d.ctypes.data, d.shape
+        if len(shape) != 3 or shape[0] != shape[1]:
+            raise ValueError("distogram must be [L][L][n_bins]")
+        e = np.ascontiguousarray(bin_edges, dtype=np.float32)
+        if e.shape != (shape[2] + 1,):
+            raise ValueError("bin_edges must be [n_bins + 1]")
+        self.L, self.n_bins = int(shape[0]), int(shape[2])
+        self.n = 2 * self.L
+        self.options = options
+        _check(lib().amh_create(C.byref(self._h), self.L, 0, dptr, e.ctypes.data, self.n_bins,
+                                C.byref(options) if options is not None else None, _stream_ptr(stream)))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().amh_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- amh_energy / amh_energy_local / amh_coords ---------------------------------------------
+    def energy(self, states, stream=None):
+        torch = _torch()
+        s = _dev(states, torch.float32, "states").reshape(-1, self.n)
+        out = torch.empty(s.shape[0], dtype=torch.float32, device="cuda")
+        _check(lib().amh_energy(self._h, s.data_ptr(), s.shape[0], out.data_ptr(), _stream_ptr(stream)))
+        return out
+
+    def energy_host(self, states: np.ndarray) -> np.ndarray:
+        s = np.ascontiguousarray(states, dtype=np.float32).reshape(-1, self.n)
+        out = np.empty(s.shape[0], np.float32)
+        _check(lib().amh_energy_host(self._h, s.ctypes.data, s.shape[0], out.ctypes.data, _stream_ptr()))
+        return out
+
+    def energy_local(self, states, k: int, window: int, stream=None):
+        torch = _torch()
+        s = _dev(states, torch.float32, "states").reshape(-1, self.n)
+        out = torch.empty(s.shape[0], dtype=torch.float32, device="cuda")
+        _check(lib().amh_energy_local(self._h, s.data_ptr(), s.shape[0], int(k), int(window), out.data_ptr(),
+                                      _stream_ptr(stream)))
+        return out
+
+    def coords(self, states, atoms: bool = False, stream=None):
+        """C-beta fp32 [B][L][3]; with atoms=True also fp64 [B][L][4][3] (N, CA, C, CB)."""
+        torch = _torch()
+        s = _dev(states, torch.float32, "states").reshape(-1, self.n)
+        B = s.shape[0]
+        cb = torch.empty((B, self.L, 3), dtype=torch.float32, device="cuda")
+        at = torch.empty((B, self.L, 4, 3), dtype=torch.float64, device="cuda") if atoms else None
+        _check(lib().amh_coords(self._h, s.data_ptr(), B, cb.data_ptr(), at.data_ptr() if atoms else None,
+                                _stream_ptr(stream)))
+        return (cb, at) if atoms else cb
+
+    def launch_info(self, B: int) -> dict:
+        v = [C.c_int() for _ in range(4)]
+        _check(lib().amh_launch_info(self._h, int(B), *[C.byref(x) for x in v]))
+        return dict(threads_per_chain=v[0].value, smem_bytes=v[1].value, ctas_per_sm=v[2].value, n_sm=v[3].value)
+
+    # ---- amh_run ---------------------------------------------------------------------------------
+    @staticmethod
+    def _structs(n_global, n_local, window, global_first, t_start, t_end, ramp_sweeps, per_chain_T_ptr,
+                 prop_mode, grid):
+        return (_Schedule(n_global, n_local, window, int(bool(global_first))),
+                _Temperature(t_start, t_end, ramp_sweeps, per_chain_T_ptr),
+                _Proposal(prop_mode, grid))
+
+    def run(self, states, n_sweeps: int, *, n_global=1, n_local=10, window=8, global_first=True,
+            t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
+            seed=1, chain_offset=0, sweep_offset=0, trace_steps=0, energy_threshold=None,
+            want=("energy", "best_energy", "best_state", "n_accept_local", "n_accept_global"), stream=None):
+        """amh_run on a DEVICE batch; `states` (torch.float32 [B][n], cuda) is updated in place.
+        Returns a dict of device tensors for the outputs named in `want` (+ traces, first_hit_sweep)."""
+        torch = _torch()
+        if not (isinstance(states, torch.Tensor) and states.is_cuda and states.dtype == torch.float32
+                and states.is_contiguous()):
+            raise ValueError("states must be a contiguous cuda float32 tensor (it is updated in place)")
+        s = states.view(-1, self.n)
+        B = s.shape[0]
+        r = {}
+        o = _Outputs()
+        f32, u64 = torch.float32, torch.int64
+
+        def alloc(name, shape, dtype):
+            r[name] = torch.empty(shape, dtype=dtype, device="cuda")
+            return r[name].data_ptr()
+        if "energy" in want: o.energy = alloc("energy", (B,), f32)
+        if "best_energy" in want: o.best_energy = alloc("best_energy", (B,), f32)
+        if "best_state" in want: o.best_state = alloc("best_state", (B, self.n), f32)
+        if "n_accept_local" in want: o.n_accept_local = alloc("n_accept_local", (B,), u64)
+        if "n_accept_global" in want: o.n_accept_global = alloc("n_accept_global", (B,), u64)
+        if energy_threshold is not None:
+            o.first_hit_sweep = alloc("first_hit_sweep", (1,), u64)
+            o.energy_threshold = float(energy_threshold)
+        if trace_steps:
+            o.trace_steps = int(trace_steps)
+            o.trace_prop = alloc("trace_prop", (B, trace_steps), f32)
+            o.trace_dE = alloc("trace_dE", (B, trace_steps), torch.float64)
+            o.trace_acc = alloc("trace_acc", (B, trace_steps), torch.uint8)
+        pct = None
+        if per_chain_T is not None:
+            pct = _dev(per_chain_T, f32, "per_chain_T")
+            if pct.numel() != B:
+                raise ValueError("per_chain_T must have B entries")
+        sc, tp, pr = self._structs(n_global, n_local, window, global_first, t_start, t_end, ramp_sweeps,
+                                   pct.data_ptr() if pct is not None else None, prop_mode, grid)
+        _check(lib().amh_run(self._h, s.data_ptr(), B, int(n_sweeps), int(sweep_offset), int(chain_offset),
+                             C.byref(sc), C.byref(tp), C.byref(pr), int(seed), C.byref(o), _stream_ptr(stream)))
+        r["_keepalive"] = pct
+        return r
+
+    def run_host(self, states: np.ndarray, n_sweeps: int, *, n_global=1, n_local=10, window=8, global_first=True,
+                 t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
+                 seed=1, chain_offset=0, sweep_offset=0, trace_steps=0, energy_threshold=None,
+                 want=("energy", "best_energy")):
+        """amh_run_host: HOST numpy buffers in and out (states updated in place); synchronous."""
+        if not (isinstance(states, np.ndarray) and states.dtype == np.float32 and states.flags.c_contiguous):
+            raise ValueError("states must be a C-contiguous float32 numpy array (it is updated in place)")
+        s = states.reshape(-1, self.n)
+        B = s.shape[0]
+        r = {}
+        o = _Outputs()
+
+        def alloc(name, shape, dtype):
+            r[name] = np.empty(shape, dtype=dtype)
+            return r[name].ctypes.data
+        if "energy" in want: o.energy = alloc("energy", (B,), np.float32)
+        if "best_energy" in want: o.best_energy = alloc("best_energy", (B,), np.float32)
+        if "best_state" in want: o.best_state = alloc("best_state", (B, self.n), np.float32)
+        if "n_accept_local" in want: o.n_accept_local = alloc("n_accept_local", (B,), np.uint64)
+        if "n_accept_global" in want: o.n_accept_global = alloc("n_accept_global", (B,), np.uint64)
+        if energy_threshold is not None:
+            o.first_hit_sweep = alloc("first_hit_sweep", (1,), np.int64)
+            o.energy_threshold = float(energy_threshold)
+        if trace_steps:
+            o.trace_steps = int(trace_steps)
+            o.trace_prop = alloc("trace_prop", (B, trace_steps), np.float32)
+            o.trace_dE = alloc("trace_dE", (B, trace_steps), np.float64)
+            o.trace_acc = alloc("trace_acc", (B, trace_steps), np.uint8)
+        pct = None
+        if per_chain_T is not None:
+            pct = np.ascontiguousarray(per_chain_T, dtype=np.float32)
+        sc, tp, pr = self._structs(n_global, n_local, window, global_first, t_start, t_end, ramp_sweeps,
+                                   pct.ctypes.data if pct is not None else None, prop_mode, grid)
+        _check(lib().amh_run_host(self._h, s.ctypes.data, B, int(n_sweeps), int(sweep_offset), int(chain_offset),
+                                  C.byref(sc), C.byref(tp), C.byref(pr), int(seed), C.byref(o), _stream_ptr()))
+        return r

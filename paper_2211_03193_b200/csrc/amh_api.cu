@@ -1,0 +1,442 @@
+// amh_api.cu - host side of the C ABI declared in include/amh.h: argument checks, the geometry
+// constants of the bond-frame recursion, launches.  No arithmetic of the method runs on the host
+// except those constants (closed forms of the ideal bond geometry, R1-R3).
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "../../include/amh.h"
+#include "amh_kernels.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+amh_status fail(amh_status st, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+#define AMH_CUDA(call)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess)                                                                      \
+            return fail(e_ == cudaErrorMemoryAllocation ? AMH_ERR_OOM : AMH_ERR_CUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                    \
+    } while (0)
+
+// Mplus(ang, tor, len) of DESIGN.md "Geometry": the bond frame reached by one NeRF placement
+amh::Xf mplus(double ang, double tor, double len)
+{
+    const double ca = std::cos(ang), sa = std::sin(ang), ct = std::cos(tor), st = std::sin(tor);
+    amh::Xf M;
+    M.r[0] = -ca;     M.r[1] = -sa;      M.r[2] = 0.0;
+    M.r[3] = sa * ct; M.r[4] = -ca * ct; M.r[5] = -st;
+    M.r[6] = sa * st; M.r[7] = -ca * st; M.r[8] = ct;
+    M.t[0] = len * M.r[0]; M.t[1] = len * M.r[3]; M.t[2] = len * M.r[6];
+    return M;
+}
+
+}  // namespace
+
+struct amh_ctx {
+    amh::DevModel m;
+    amh_options opt;
+    float *E = nullptr;
+    int device = 0, n_sm = 0, max_smem = 0;
+    // staging for the *_host calls (grow-only)
+    void *stage = nullptr;
+    size_t stage_bytes = 0;
+    unsigned long long *first_hit_dev = nullptr;   // scratch for amh_run's first-hit reduction
+};
+
+extern "C" {
+
+const char *amh_last_error(void) { return g_err; }
+const char *amh_version(void) { return "amh-b200 0.1 (sm_100a)"; }
+
+amh_status amh_default_options(amh_options *o)
+{
+    if (!o) return fail(AMH_ERR_INVALID_ARG, "amh_default_options: opt is NULL");
+    o->len_n_ca = 1.458; o->len_ca_c = 1.525; o->len_c_n = 1.329;
+    o->ang_n_ca_c = 111.2 * M_PI / 180.0;
+    o->ang_ca_c_n = 116.2 * M_PI / 180.0;
+    o->ang_c_n_ca = 121.7 * M_PI / 180.0;
+    o->omega = M_PI;
+    o->cb_len = 1.522; o->cb_ang = 1.927; o->cb_dih = -2.143;
+    o->eps = 1e-8;
+    o->min_sep = 3;
+    o->warps_per_chain = 0;
+    return AMH_OK;
+}
+
+amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *distogram,
+                      const float *bin_edges, int n_bins, const amh_options *opt, void *cuda_stream)
+{
+    if (!out) return fail(AMH_ERR_INVALID_ARG, "amh_create: out is NULL");
+    *out = nullptr;
+    if (param == AMH_PARAM_TR5) return fail(AMH_ERR_UNSUPPORTED, "amh_create: AMH_PARAM_TR5 (config 3) is not built");
+    if (param != AMH_PARAM_PHI_PSI) return fail(AMH_ERR_INVALID_ARG, "amh_create: unknown parameterisation %d", (int)param);
+    if (n_res < 1) return fail(AMH_ERR_INVALID_ARG, "amh_create: n_res = %d < 1", n_res);
+    if (n_bins < 2) return fail(AMH_ERR_INVALID_ARG, "amh_create: n_bins = %d < 2", n_bins);
+    if (!distogram || !bin_edges) return fail(AMH_ERR_INVALID_ARG, "amh_create: distogram / bin_edges is NULL");
+    amh_options o;
+    amh_default_options(&o);
+    if (opt) o = *opt;
+    if (o.min_sep < 1) return fail(AMH_ERR_INVALID_ARG, "amh_create: min_sep = %d < 1", o.min_sep);
+    if (!(o.eps >= 0.0)) return fail(AMH_ERR_INVALID_ARG, "amh_create: eps < 0");
+    {
+        const int w = o.warps_per_chain;
+        if (!(w == 0 || w == 1 || w == 2 || w == 4 || w == 8 || w == 16))
+            return fail(AMH_ERR_INVALID_ARG, "amh_create: warps_per_chain = %d not in {0,1,2,4,8,16}", w);
+    }
+    for (int b = 0; b <= n_bins; ++b)
+        if (!std::isfinite(bin_edges[b])) return fail(AMH_ERR_INVALID_ARG, "amh_create: bin edge %d is not finite", b);
+    const double e0 = bin_edges[0], e1 = bin_edges[n_bins];
+    const double delta = (e1 - e0) / n_bins;
+    if (!(delta > 0.0)) return fail(AMH_ERR_INVALID_ARG, "amh_create: bin edges do not increase");
+    for (int b = 0; b < n_bins; ++b) {
+        const double w = (double)bin_edges[b + 1] - (double)bin_edges[b];
+        if (!(w > 0.0)) return fail(AMH_ERR_INVALID_ARG, "amh_create: bin edges do not increase at %d", b);
+        if (std::fabs(w - delta) > 1e-5 * delta)
+            return fail(AMH_ERR_UNSUPPORTED, "amh_create: bins are not evenly spaced (bin %d: %g vs %g)", b, w, delta);
+    }
+
+    amh_ctx *c = new (std::nothrow) amh_ctx;
+    if (!c) return fail(AMH_ERR_OOM, "amh_create: host allocation failed");
+    c->opt = o;
+    cudaError_t e = cudaGetDevice(&c->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device);
+    if (e != cudaSuccess) { delete c; return fail(AMH_ERR_CUDA, "amh_create: no usable CUDA device: %s", cudaGetErrorString(e)); }
+
+    amh::DevModel &m = c->m;
+    m.L = n_res; m.nb = n_bins; m.min_sep = o.min_sep; m.n = 2 * n_res;
+    m.c0 = (float)(e0 + 0.5 * delta);
+    m.inv_delta = (float)(1.0 / delta);
+    m.tmax = (float)(n_bins - 1);
+    m.A = mplus(o.ang_n_ca_c, 0.0, o.len_ca_c);
+    m.W = mplus(o.ang_c_n_ca, o.omega, o.len_n_ca);
+    m.c2 = std::cos(o.ang_ca_c_n); m.s2 = std::sin(o.ang_ca_c_n); m.l3 = o.len_c_n;
+    // atoms in the residue's bond frame (origin CA, x along N->CA, C at torsion 0)
+    m.loc[0][0] = -o.len_n_ca; m.loc[0][1] = 0.0; m.loc[0][2] = 0.0;
+    m.loc[1][0] = 0.0; m.loc[1][1] = 0.0; m.loc[1][2] = 0.0;
+    m.loc[2][0] = -o.len_ca_c * std::cos(o.ang_n_ca_c); m.loc[2][1] = o.len_ca_c * std::sin(o.ang_n_ca_c); m.loc[2][2] = 0.0;
+    m.loc[3][0] = -o.cb_len * std::cos(o.cb_ang);
+    m.loc[3][1] = o.cb_len * std::sin(o.cb_ang) * std::cos(o.cb_dih);
+    m.loc[3][2] = o.cb_len * std::sin(o.cb_ang) * std::sin(o.cb_dih);
+    m.h0x = o.len_n_ca;
+
+    if (amh::sweep_smem_bytes(n_res) > (size_t)c->max_smem) {
+        delete c;
+        return fail(AMH_ERR_UNSUPPORTED, "amh_create: L = %d needs %zu B of shared memory per chain, device allows %d",
+                    n_res, amh::sweep_smem_bytes(n_res), c->max_smem);
+    }
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long count = (long long)n_res * n_res * n_bins;
+    float *p_dev = nullptr;
+    int *bad_dev = nullptr;
+    cudaPointerAttributes at;
+    bool on_device = (cudaPointerGetAttributes(&at, distogram) == cudaSuccess) &&
+                     (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged);
+    cudaGetLastError();
+    auto cleanup = [&]() {
+        if (p_dev) cudaFree(p_dev);
+        if (bad_dev) cudaFree(bad_dev);
+        if (c->E) cudaFree(c->E);
+        if (c->first_hit_dev) cudaFree(c->first_hit_dev);
+        delete c;
+    };
+#define AMH_CUDA_C(call)                                                                           \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            cleanup();                                                                             \
+            return fail(e_ == cudaErrorMemoryAllocation ? AMH_ERR_OOM : AMH_ERR_CUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                   \
+        }                                                                                          \
+    } while (0)
+    AMH_CUDA_C(cudaMalloc(&c->E, sizeof(float) * (size_t)count));
+    AMH_CUDA_C(cudaMalloc(&bad_dev, sizeof(int)));
+    AMH_CUDA_C(cudaMalloc(&c->first_hit_dev, sizeof(unsigned long long)));
+    AMH_CUDA_C(cudaMemsetAsync(bad_dev, 0, sizeof(int), st));
+    const float *src = distogram;
+    if (!on_device) {
+        AMH_CUDA_C(cudaMalloc(&p_dev, sizeof(float) * (size_t)count));
+        AMH_CUDA_C(cudaMemcpyAsync(p_dev, distogram, sizeof(float) * (size_t)count, cudaMemcpyHostToDevice, st));
+        src = p_dev;
+    }
+    {
+        const int threads = 256;
+        const int blocks = (int)std::min<long long>((count + threads - 1) / threads, (long long)c->n_sm * 16);
+        amh::table_kernel<<<blocks, threads, 0, st>>>(src, c->E, count, o.eps, bad_dev);
+        AMH_CUDA_C(cudaGetLastError());
+    }
+    int bad = 0;
+    AMH_CUDA_C(cudaMemcpyAsync(&bad, bad_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
+    AMH_CUDA_C(cudaStreamSynchronize(st));
+    if (bad) { cleanup(); return fail(AMH_ERR_INVALID_ARG, "amh_create: the distogram holds a negative, NaN or infinite value"); }
+    cudaFree(bad_dev); bad_dev = nullptr;
+    if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
+    m.E = c->E;
+    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+    AMH_CUDA_C(cudaFuncSetAttribute(amh::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+#undef AMH_CUDA_C
+    *out = c;
+    return AMH_OK;
+}
+
+amh_status amh_destroy(amh_ctx *c)
+{
+    if (!c) return AMH_OK;
+    cudaDeviceSynchronize();
+    if (c->E) cudaFree(c->E);
+    if (c->stage) cudaFree(c->stage);
+    if (c->first_hit_dev) cudaFree(c->first_hit_dev);
+    delete c;
+    return AMH_OK;
+}
+
+static amh_status launch_energy(amh_ctx *c, const float *states, long long B, int k, int window, float *out, cudaStream_t st)
+{
+    if (B == 0) return AMH_OK;
+    const size_t smem = sizeof(double) * 32 + sizeof(float) * 3 * (size_t)c->m.L;
+    const int blocks = (int)std::min<long long>(B, (long long)c->n_sm * 64);
+    amh::energy_kernel<<<blocks, 128, smem, st>>>(c->m, states, B, k, window, out);
+    AMH_CUDA(cudaGetLastError());
+    return AMH_OK;
+}
+
+amh_status amh_energy(amh_ctx *c, const float *states, long long B, float *energy_out, void *cuda_stream)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_energy: ctx is NULL");
+    if (B < 0) return fail(AMH_ERR_INVALID_ARG, "amh_energy: B = %lld < 0", B);
+    if (B > 0 && (!states || !energy_out)) return fail(AMH_ERR_INVALID_ARG, "amh_energy: states / energy_out is NULL");
+    return launch_energy(c, states, B, -1, 0, energy_out, (cudaStream_t)cuda_stream);
+}
+
+amh_status amh_energy_local(amh_ctx *c, const float *states, long long B, int k, int window, float *energy_out,
+                            void *cuda_stream)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_energy_local: ctx is NULL");
+    if (B < 0) return fail(AMH_ERR_INVALID_ARG, "amh_energy_local: B = %lld < 0", B);
+    if (k < 0 || k >= c->m.n) return fail(AMH_ERR_INVALID_ARG, "amh_energy_local: k = %d outside [0, %d)", k, c->m.n);
+    if (window < 0) return fail(AMH_ERR_INVALID_ARG, "amh_energy_local: window = %d < 0", window);
+    if (B > 0 && (!states || !energy_out)) return fail(AMH_ERR_INVALID_ARG, "amh_energy_local: states / energy_out is NULL");
+    return launch_energy(c, states, B, k, window, energy_out, (cudaStream_t)cuda_stream);
+}
+
+amh_status amh_coords(amh_ctx *c, const float *states, long long B, float *cb_out, double *atoms_out, void *cuda_stream)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_coords: ctx is NULL");
+    if (B < 0) return fail(AMH_ERR_INVALID_ARG, "amh_coords: B = %lld < 0", B);
+    if (B == 0 || (!cb_out && !atoms_out)) return AMH_OK;
+    if (!states) return fail(AMH_ERR_INVALID_ARG, "amh_coords: states is NULL");
+    const int wpb = 4;
+    const long long blocks = (B + wpb - 1) / wpb;
+    if (blocks > 0x7fffffffLL) return fail(AMH_ERR_INVALID_ARG, "amh_coords: B too large");
+    amh::coords_kernel<<<(int)blocks, 32 * wpb, 0, (cudaStream_t)cuda_stream>>>(c->m, states, B, cb_out, atoms_out);
+    AMH_CUDA(cudaGetLastError());
+    return AMH_OK;
+}
+
+// warps per chain-CTA: enough lanes for the O(L^2/6) pairs of a global proposal, without starving
+// the SM of resident chains
+static int choose_warps(const amh_ctx *c, long long B)
+{
+    if (c->opt.warps_per_chain > 0) return c->opt.warps_per_chain;
+    const int L = c->m.L;
+    const size_t smem = amh::sweep_smem_bytes(L) + 1024;
+    const long long by_smem = std::max<long long>(1, (long long)(228 * 1024) / (long long)smem);
+    const long long resident = std::min<long long>(B, by_smem * c->n_sm);
+    const long long per_sm = std::max<long long>(1, (resident + c->n_sm - 1) / c->n_sm);
+    const long long by_occ = std::max<long long>(1, 48 / per_sm);
+    const long long by_work = std::max<long long>(1, ((long long)L * L / 6) / (32 * 8));
+    long long w = std::min(by_occ, by_work);
+    int p = 1;
+    while (2 * p <= w && p < 16) p *= 2;
+    return p;
+}
+
+amh_status amh_launch_info(amh_ctx *c, long long B, int *threads_per_chain, int *smem_bytes, int *ctas_per_sm, int *n_sm)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_launch_info: ctx is NULL");
+    const int w = choose_warps(c, std::max<long long>(B, 1));
+    const size_t smem = amh::sweep_smem_bytes(c->m.L);
+    if (threads_per_chain) *threads_per_chain = 32 * w;
+    if (smem_bytes) *smem_bytes = (int)smem;
+    if (n_sm) *n_sm = c->n_sm;
+    if (ctas_per_sm) {
+        int nb = 0;
+        AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::sweep_kernel, 32 * w, smem));
+        *ctas_per_sm = nb;
+    }
+    return AMH_OK;
+}
+
+static amh_status check_run(const amh_ctx *c, const float *states, long long B, long long n_sweeps, long long sweep_offset,
+                            const amh_schedule *sc, const amh_temperature *tp, const amh_proposal *pr,
+                            const amh_outputs *out)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_run: ctx is NULL");
+    if (B < 0 || B > 0x7fffffffLL) return fail(AMH_ERR_INVALID_ARG, "amh_run: B = %lld out of range", B);
+    if (B > 0 && !states) return fail(AMH_ERR_INVALID_ARG, "amh_run: states is NULL");
+    if (n_sweeps < 0 || sweep_offset < 0) return fail(AMH_ERR_INVALID_ARG, "amh_run: n_sweeps / sweep_offset < 0");
+    if (!sc || !tp) return fail(AMH_ERR_INVALID_ARG, "amh_run: schedule / temperature is NULL");
+    if (sc->n_global < 0 || sc->n_local < 0 || sc->n_global + sc->n_local < 1)
+        return fail(AMH_ERR_INVALID_ARG, "amh_run: schedule needs n_global, n_local >= 0 and n_global + n_local >= 1");
+    if (sc->window < 0) return fail(AMH_ERR_INVALID_ARG, "amh_run: window = %d < 0", sc->window);
+    if (!tp->per_chain_T && !(tp->t_start > 0.0 && tp->t_end > 0.0 && std::isfinite(tp->t_start) && std::isfinite(tp->t_end)))
+        return fail(AMH_ERR_INVALID_ARG, "amh_run: temperatures must be finite and > 0");
+    if (pr) {
+        if (pr->mode == 2) return fail(AMH_ERR_UNSUPPORTED, "amh_run: Gaussian proposals are not built (DESIGN.md NEXT-1)");
+        if (pr->mode != AMH_PROP_UNIFORM && pr->mode != AMH_PROP_GRID) return fail(AMH_ERR_INVALID_ARG, "amh_run: unknown proposal mode %d", pr->mode);
+        if (pr->mode == AMH_PROP_GRID && (pr->grid < 1 || pr->grid > (1 << 20))) return fail(AMH_ERR_INVALID_ARG, "amh_run: grid = %d out of range", pr->grid);
+    }
+    if (out && out->trace_steps < 0) return fail(AMH_ERR_INVALID_ARG, "amh_run: trace_steps < 0");
+    return AMH_OK;
+}
+
+amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, long long sweep_offset,
+                   long long chain_offset, const amh_schedule *sc, const amh_temperature *tp,
+                   const amh_proposal *pr, unsigned long long seed, const amh_outputs *out, void *cuda_stream)
+{
+    amh_status stt = check_run(c, states, B, n_sweeps, sweep_offset, sc, tp, pr, out);
+    if (stt != AMH_OK) return stt;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    amh::RunArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.states = states; a.B = B; a.n_sweeps = n_sweeps; a.sweep_offset = sweep_offset; a.chain_offset = chain_offset;
+    a.n_global = sc->n_global; a.n_local = sc->n_local; a.window = sc->window; a.global_first = sc->global_first ? 1 : 0;
+    a.t_start = tp->t_start; a.t_end = tp->t_end; a.ramp_sweeps = tp->ramp_sweeps; a.per_chain_T = tp->per_chain_T;
+    a.prop_mode = pr ? pr->mode : AMH_PROP_UNIFORM; a.grid = pr ? pr->grid : 0;
+    a.seed = seed;
+    if (out) {
+        a.energy = out->energy; a.best_energy = out->best_energy; a.best_state = out->best_state;
+        a.n_accept_local = out->n_accept_local; a.n_accept_global = out->n_accept_global;
+        a.first_hit = reinterpret_cast<unsigned long long *>(out->first_hit_sweep);
+        a.energy_threshold = out->energy_threshold;
+        a.trace_steps = out->trace_steps; a.trace_prop = out->trace_prop; a.trace_dE = out->trace_dE; a.trace_acc = out->trace_acc;
+        if (a.first_hit) AMH_CUDA(cudaMemsetAsync(a.first_hit, 0xFF, sizeof(unsigned long long), st));   // -1 = none
+    }
+    if (B == 0) return AMH_OK;
+    const int w = choose_warps(c, B);
+    const size_t smem = amh::sweep_smem_bytes(c->m.L);
+    amh::sweep_kernel<<<(unsigned)B, 32 * w, smem, st>>>(c->m, a);
+    AMH_CUDA(cudaGetLastError());
+    return AMH_OK;
+}
+
+static amh_status ensure_stage(amh_ctx *c, size_t bytes)
+{
+    if (bytes <= c->stage_bytes) return AMH_OK;
+    if (c->stage) { cudaDeviceSynchronize(); cudaFree(c->stage); c->stage = nullptr; c->stage_bytes = 0; }
+    AMH_CUDA(cudaMalloc(&c->stage, bytes));
+    c->stage_bytes = bytes;
+    return AMH_OK;
+}
+
+static size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+amh_status amh_run_host(amh_ctx *c, float *states, long long B, long long n_sweeps, long long sweep_offset,
+                        long long chain_offset, const amh_schedule *sc, const amh_temperature *tp,
+                        const amh_proposal *pr, unsigned long long seed, const amh_outputs *out, void *cuda_stream)
+{
+    amh_status stt = check_run(c, states, B, n_sweeps, sweep_offset, sc, tp, pr, out);
+    if (stt != AMH_OK) return stt;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)c->m.n, b = (size_t)B;
+    const size_t ts = out ? (size_t)out->trace_steps : 0;
+    // carve the staging arena
+    size_t off = 0;
+    auto take = [&](bool want, size_t bytes) { size_t o = off; if (want) off += up256(bytes); return o; };
+    const size_t o_states = take(true, b * n * 4);
+    const size_t o_T = take(tp->per_chain_T != nullptr, b * 4);
+    const size_t o_e = take(out && out->energy, b * 4);
+    const size_t o_be = take(out && out->best_energy, b * 4);
+    const size_t o_bs = take(out && out->best_state, b * n * 4);
+    const size_t o_al = take(out && out->n_accept_local, b * 8);
+    const size_t o_ag = take(out && out->n_accept_global, b * 8);
+    const size_t o_fh = take(out && out->first_hit_sweep, 8);
+    const size_t o_tp = take(out && out->trace_prop && ts, b * ts * 4);
+    const size_t o_td = take(out && out->trace_dE && ts, b * ts * 8);
+    const size_t o_ta = take(out && out->trace_acc && ts, b * ts);
+    stt = ensure_stage(c, off + 256);
+    if (stt != AMH_OK) return stt;
+    char *base = static_cast<char *>(c->stage);
+    AMH_CUDA(cudaMemcpyAsync(base + o_states, states, b * n * 4, cudaMemcpyHostToDevice, st));
+    amh_temperature tpd = *tp;
+    if (tp->per_chain_T) {
+        AMH_CUDA(cudaMemcpyAsync(base + o_T, tp->per_chain_T, b * 4, cudaMemcpyHostToDevice, st));
+        tpd.per_chain_T = reinterpret_cast<const float *>(base + o_T);
+    }
+    amh_outputs od;
+    std::memset(&od, 0, sizeof od);
+    if (out) {
+        od = *out;
+        od.energy = out->energy ? reinterpret_cast<float *>(base + o_e) : nullptr;
+        od.best_energy = out->best_energy ? reinterpret_cast<float *>(base + o_be) : nullptr;
+        od.best_state = out->best_state ? reinterpret_cast<float *>(base + o_bs) : nullptr;
+        od.n_accept_local = out->n_accept_local ? reinterpret_cast<unsigned long long *>(base + o_al) : nullptr;
+        od.n_accept_global = out->n_accept_global ? reinterpret_cast<unsigned long long *>(base + o_ag) : nullptr;
+        od.first_hit_sweep = out->first_hit_sweep ? reinterpret_cast<long long *>(base + o_fh) : nullptr;
+        od.trace_prop = (out->trace_prop && ts) ? reinterpret_cast<float *>(base + o_tp) : nullptr;
+        od.trace_dE = (out->trace_dE && ts) ? reinterpret_cast<double *>(base + o_td) : nullptr;
+        od.trace_acc = (out->trace_acc && ts) ? reinterpret_cast<unsigned char *>(base + o_ta) : nullptr;
+    }
+    stt = amh_run(c, reinterpret_cast<float *>(base + o_states), B, n_sweeps, sweep_offset, chain_offset, sc, &tpd, pr,
+                  seed, out ? &od : nullptr, cuda_stream);
+    if (stt != AMH_OK) return stt;
+    AMH_CUDA(cudaMemcpyAsync(states, base + o_states, b * n * 4, cudaMemcpyDeviceToHost, st));
+    if (out) {
+        if (od.energy) AMH_CUDA(cudaMemcpyAsync(out->energy, od.energy, b * 4, cudaMemcpyDeviceToHost, st));
+        if (od.best_energy) AMH_CUDA(cudaMemcpyAsync(out->best_energy, od.best_energy, b * 4, cudaMemcpyDeviceToHost, st));
+        if (od.best_state) AMH_CUDA(cudaMemcpyAsync(out->best_state, od.best_state, b * n * 4, cudaMemcpyDeviceToHost, st));
+        if (od.n_accept_local) AMH_CUDA(cudaMemcpyAsync(out->n_accept_local, od.n_accept_local, b * 8, cudaMemcpyDeviceToHost, st));
+        if (od.n_accept_global) AMH_CUDA(cudaMemcpyAsync(out->n_accept_global, od.n_accept_global, b * 8, cudaMemcpyDeviceToHost, st));
+        if (od.first_hit_sweep) AMH_CUDA(cudaMemcpyAsync(out->first_hit_sweep, od.first_hit_sweep, 8, cudaMemcpyDeviceToHost, st));
+        if (od.trace_prop) AMH_CUDA(cudaMemcpyAsync(out->trace_prop, od.trace_prop, b * ts * 4, cudaMemcpyDeviceToHost, st));
+        if (od.trace_dE) AMH_CUDA(cudaMemcpyAsync(out->trace_dE, od.trace_dE, b * ts * 8, cudaMemcpyDeviceToHost, st));
+        if (od.trace_acc) AMH_CUDA(cudaMemcpyAsync(out->trace_acc, od.trace_acc, b * ts, cudaMemcpyDeviceToHost, st));
+    }
+    AMH_CUDA(cudaStreamSynchronize(st));
+    return AMH_OK;
+}
+
+amh_status amh_energy_host(amh_ctx *c, const float *states, long long B, float *energy_out, void *cuda_stream)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_energy_host: ctx is NULL");
+    if (B < 0) return fail(AMH_ERR_INVALID_ARG, "amh_energy_host: B = %lld < 0", B);
+    if (B == 0) return AMH_OK;
+    if (!states || !energy_out) return fail(AMH_ERR_INVALID_ARG, "amh_energy_host: states / energy_out is NULL");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t bytes = (size_t)B * c->m.n * 4;
+    amh_status stt = ensure_stage(c, up256(bytes) + up256((size_t)B * 4));
+    if (stt != AMH_OK) return stt;
+    char *base = static_cast<char *>(c->stage);
+    float *e_dev = reinterpret_cast<float *>(base + up256(bytes));
+    AMH_CUDA(cudaMemcpyAsync(base, states, bytes, cudaMemcpyHostToDevice, st));
+    stt = launch_energy(c, reinterpret_cast<const float *>(base), B, -1, 0, e_dev, st);
+    if (stt != AMH_OK) return stt;
+    AMH_CUDA(cudaMemcpyAsync(energy_out, e_dev, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+    AMH_CUDA(cudaStreamSynchronize(st));
+    return AMH_OK;
+}
+
+amh_status amh_philox_test(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long count, void *cuda_stream)
+{
+    if (count < 0 || (count > 0 && (!ctr || !key || !out))) return fail(AMH_ERR_INVALID_ARG, "amh_philox_test: bad arguments");
+    if (count == 0) return AMH_OK;
+    amh::philox_test_kernel<<<(unsigned)((count + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(ctr, key, out, count);
+    AMH_CUDA(cudaGetLastError());
+    return AMH_OK;
+}
+
+}  // extern "C"

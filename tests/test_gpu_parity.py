@@ -1,0 +1,381 @@
+"""Parity of the CUDA path (through the C ABI of include/amh.h) against the fp64 oracle, element by
+element on the same seeded inputs.  Bars (BASELINE.json north_star): coordinates 1e-4 A, energies
+1e-5 relative, accept/reject trajectories identical over the first 1000 steps of every chain of
+config 0 except at logged near-ties |log u + dE/T| < 1e-4; integer work (Philox, proposal values,
+counters) bit-exact.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import amh_inputs as gi
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def amh():
+    import paper_2211_03193_b200 as pkg
+    pkg.lib()           # raises if the extension is missing: no fallback
+    return pkg
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gpu_model(amh, synth):
+    cache = {}
+
+    def make(L, cfg_seed=1000, **opt):
+        key = (L, cfg_seed, tuple(sorted(opt.items())))
+        if key not in cache:
+            ref, p, edges, m = synth(L, cfg_seed)
+            cache[key] = amh.AMH(p, edges, amh.default_options(**opt) if opt else None)
+        return cache[key]
+    return make
+
+
+def states_for(L, seed, B):
+    """random states + the all-180 state + an alpha-helix (compact: exercises the steep bins)"""
+    s = gi.initial_states(B, 2 * L, seed)
+    s[-1] = np.float32(math.pi)
+    if B > 1:
+        s[-2, 0::2] = np.float32(math.radians(-57.8)); s[-2, 1::2] = np.float32(math.radians(-47.0))
+    return s
+
+
+# ---------------------------------------------------------------------------------------------
+def test_device_philox_matches_kat_and_oracle(amh, orc):
+    kat = []
+    for line in open(__file__.rsplit("/", 1)[0] + "/golden/philox4x32_10_kat.txt"):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = [int(x, 16) for x in line.split()]
+        kat.append((w[:4], w[4:6], w[6:]))
+    rng = np.random.default_rng(0)
+    ctr = np.array([k[0] for k in kat] + rng.integers(0, 2 ** 32, (500, 4)).tolist(), dtype=np.uint32)
+    key = np.array([k[1] for k in kat] + rng.integers(0, 2 ** 32, (500, 2)).tolist(), dtype=np.uint32)
+    out = amh.philox4x32_10(ctr, key)
+    for q, k in enumerate(kat):
+        assert out[q].tolist() == k[2]
+    for q in range(len(kat), len(ctr), 7):
+        assert np.array_equal(out[q], orc.philox4x32_10(ctr[q], key[q]))
+
+
+@pytest.mark.parametrize("L", [1, 2, 3, 4, 33, 64, 128, 256, 600])
+def test_coords_parity(amh, orc, torch, synth, gpu_model, L):
+    g = gpu_model(L)
+    s = states_for(L, 7, 6)
+    cb, at = g.coords(torch.from_numpy(s).cuda(), atoms=True)
+    cb, at = cb.cpu().numpy(), at.cpu().numpy()
+    worst64 = worst32 = worstD = 0.0
+    for b in range(len(s)):
+        N, CA, C, CB = orc.coords(s[b])
+        want = np.stack([N, CA, C, CB], axis=1)
+        worst64 = max(worst64, float(np.abs(at[b] - want).max()))
+        # fp32 output: 1e-4 A plus the representation error of fp32 at that magnitude (the all-180
+        # chain reaches 2280 A at L = 600, where one fp32 ulp is 2.4e-4 A)
+        tol = 1e-4 + np.abs(CB) * 2.0 ** -24
+        assert np.all(np.abs(cb[b] - CB) <= tol)
+        worst32 = max(worst32, float((np.abs(cb[b] - CB) - np.abs(CB) * 2.0 ** -24).max()))
+        if L > 1:
+            Dg = np.linalg.norm(at[b][:, None, 3] - at[b][None, :, 3], axis=-1)
+            Do = np.linalg.norm(CB[:, None] - CB[None], axis=-1)
+            worstD = max(worstD, float(np.abs(Dg - Do).max()))
+    assert worst64 < 1e-9          # the fp64 scan agrees with the sequential fp64 NeRF far below the bar
+    assert worstD < 1e-9
+    print("L=%d  max|atoms64 - oracle| = %.3g A, distance matrix %.3g A" % (L, worst64, worstD))
+
+
+@pytest.mark.parametrize("L,cfg_seed", [(1, 1000), (3, 1000), (4, 1000), (33, 1000), (64, 1000), (128, 1001),
+                                        (256, 1002), (600, 1004)])
+def test_energy_parity(amh, orc, torch, synth, gpu_model, L, cfg_seed):
+    ref, p, edges, m = synth(L, cfg_seed)
+    g = gpu_model(L, cfg_seed)
+    B = 1003 if L <= 128 else (300 if L == 256 else 40)
+    s = np.concatenate([states_for(L, 11, B), ref[None]])
+    e = g.energy(torch.from_numpy(s).cuda()).cpu().numpy().astype(np.float64)
+    want = m.energy(s)
+    if L < 4:
+        assert np.all(e == 0.0) and np.all(want == 0.0)
+        return
+    rel = np.abs(e - want) / np.abs(want)
+    assert rel.max() < 1e-5, rel.max()
+    print("L=%d  energy rel err max %.3g" % (L, rel.max()))
+    # host-buffer entry point gives the same numbers
+    eh = g.energy_host(s[:17])
+    assert np.array_equal(eh.astype(np.float64), e[:17])
+
+
+def test_energy_local_parity(amh, orc, torch, synth, gpu_model):
+    L = 64
+    ref, p, edges, m = synth(L, 1000)
+    g = gpu_model(L, 1000)
+    s = states_for(L, 13, 9)
+    sd = torch.from_numpy(s).cuda()
+    for k, w in ((0, 8), (1, 8), (17, 8), (64, 12), (126, 8), (127, 3), (40, 0), (40, 1), (40, 200)):
+        e = g.energy_local(sd, k, w).cpu().numpy().astype(np.float64)
+        want = np.array([m.energy_local(x, k, w) for x in s])
+        assert np.all(np.abs(e - want) <= 1e-5 * np.maximum(np.abs(want), 1.0))
+    full = g.energy(sd).cpu().numpy()
+    assert np.array_equal(g.energy_local(sd, 5, L).cpu().numpy(), full)     # w >= L-1 is V
+
+
+def test_min_sep_option(amh, orc, torch, synth):
+    L = 24
+    ref, p, edges, _ = synth(L, 1000)
+    s = gi.initial_states(5, 2 * L, 3)
+    for ms in (1, 2, 5):
+        m = orc.Model(p, edges, orc.default_geom(min_sep=ms))
+        g = amh.AMH(p, edges, amh.default_options(min_sep=ms))
+        e = g.energy(torch.from_numpy(s).cuda()).cpu().numpy()
+        assert np.allclose(e, m.energy(s), rtol=1e-5)
+
+
+# ---------------------------------------------------------------------------------------------
+def _follow_check(m, s0, r, steps, **kw):
+    """Follow-mode protocol: the oracle replays the GPU's decisions and checks its own."""
+    acc = r["trace_acc"].cpu().numpy()
+    prop = r["trace_prop"].cpu().numpy()
+    dE = r["trace_dE"].cpu().numpy()
+    f = m.follow(s0, steps, acc, **kw)
+    assert np.array_equal(f["prop"], prop), "proposal values must be bit-identical (R5)"
+    err = np.abs(dE - f["dE"])
+    diff = acc != f["acc"]
+    near = np.abs(f["g"]) < 1e-4
+    assert np.all(near[diff]), "decisions may differ only at near-ties |g| < 1e-4: g = %s" % f["g"][diff]
+    return dict(err=err, n_diff=int(diff.sum()), n_near=int(near.sum()), f=f, acc=acc)
+
+
+@pytest.mark.parametrize("wpc", [0, 1, 4])
+def test_trajectory_parity_config0_first_1000_steps(amh, orc, torch, synth, wpc):
+    c = gi.CONFIGS[0]
+    ref, p, edges, m = synth(c.L, c.cfg_seed)
+    g = amh.AMH(p, edges, amh.default_options(warps_per_chain=wpc))
+    s0 = gi.initial_states(c.B, c.n, seed=1)
+    st = torch.from_numpy(s0.copy()).cuda()
+    steps = 1024                           # 8 full sweeps: steps 0..999 are the bar (R21), 24 more close the sweep
+    kw = dict(n_global=c.n_global, n_local=c.n_local, window=c.window, seed=1)
+    r = g.run(st, 8, trace_steps=steps, **kw)
+    chk = _follow_check(m, s0, r, steps, **kw)
+    err = chk["err"]
+    print("cfg0 wpc=%d: |dE_gpu - dE_oracle| median %.2e  p99 %.2e  max %.2e; decisions differing %d, near-ties %d of %d"
+          % (wpc, np.median(err), np.quantile(err, 0.99), err.max(), chk["n_diff"], chk["n_near"], err.size))
+    assert err.max() < 2e-3
+    assert np.quantile(err, 0.99) < 3e-4
+    # first 1000 steps = 128 global + 872 local proposals: both phases are exercised
+    # the states the kernel returns are the ones the forced replay ends in
+    assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+    # chains without any disagreement must equal the FREE-running oracle bit for bit
+    if chk["n_diff"] == 0:
+        free = m.run(s0, 8, **kw)
+        assert np.array_equal(free["states"], st.cpu().numpy())
+        assert np.array_equal(free["n_accept_local"], r["n_accept_local"].cpu().numpy())
+        assert np.array_equal(free["n_accept_global"], r["n_accept_global"].cpu().numpy())
+        e = r["energy"].cpu().numpy().astype(np.float64)
+        assert np.all(np.abs(e - free["energy"]) < 1e-5 * np.abs(free["energy"]))
+        be = r["best_energy"].cpu().numpy().astype(np.float64)
+        assert np.all(np.abs(be - free["best_energy"]) < 1e-5 * np.abs(free["best_energy"]))
+        assert np.array_equal(r["best_state"].cpu().numpy(), free["best_state"])
+
+
+@pytest.mark.parametrize("n_global,n_local,T", [(1, 0, 1.0), (0, 1, 1.0), (1, 2, 0.3), (2, 3, 4.0)])
+def test_trajectory_parity_pure_phases_and_temperatures(amh, orc, torch, synth, gpu_model, n_global, n_local, T):
+    L, B, sweeps = 48, 16, 6
+    ref, p, edges, m = synth(L, 1000)
+    g = gpu_model(L, 1000)
+    s0 = gi.initial_states(B, 2 * L, seed=5)
+    st = torch.from_numpy(s0.copy()).cuda()
+    steps = sweeps * 2 * L
+    kw = dict(n_global=n_global, n_local=n_local, window=5, seed=77, t_start=T, t_end=T, chain_offset=3)
+    r = g.run(st, sweeps, trace_steps=steps, **kw)
+    chk = _follow_check(m, s0, r, steps, **kw)
+    assert chk["err"].max() < 2e-3
+    assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+    assert 0 < chk["acc"].mean() < 1
+
+
+def test_trajectory_parity_ramp_per_chain_T_and_offset(amh, orc, torch, synth, gpu_model):
+    L, B, sweeps = 40, 8, 5
+    ref, p, edges, m = synth(L, 1000)
+    g = gpu_model(L, 1000)
+    s0 = gi.initial_states(B, 2 * L, seed=9)
+    steps = sweeps * 2 * L
+    # geometric ramp, starting mid-run
+    kw = dict(n_global=1, n_local=2, window=4, seed=5, t_start=10.0, t_end=0.1, ramp_sweeps=12, sweep_offset=4)
+    st = torch.from_numpy(s0.copy()).cuda()
+    r = g.run(st, sweeps, trace_steps=steps, **kw)
+    chk = _follow_check(m, s0, r, steps, **kw)
+    assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+    # per-chain constant temperatures (config 4's replicas)
+    T = gi.per_chain_temperature(B, 8, 0.1, 5.0)
+    kw = dict(n_global=1, n_local=2, window=4, seed=6, per_chain_T=T)
+    st = torch.from_numpy(s0.copy()).cuda()
+    r = g.run(st, sweeps, trace_steps=steps, **kw)
+    chk = _follow_check(m, s0, r, steps, **kw)
+    assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+    acc = chk["acc"].mean(axis=1)
+    assert acc[7] > acc[0]                    # the hot replica accepts more
+
+
+@pytest.mark.parametrize("L", [2, 3, 5])
+def test_tiny_chains_run(amh, orc, torch, synth, gpu_model, L):
+    # degenerate sizes: L < min_sep + 1 has no pairs (every proposal accepted); window clamps at both ends
+    ref, p, edges, m = synth(L, 1000)
+    g = gpu_model(L, 1000)
+    s0 = gi.initial_states(4, 2 * L, seed=2)
+    st = torch.from_numpy(s0.copy()).cuda()
+    kw = dict(n_global=1, n_local=1, window=8, seed=3)
+    steps = 6 * 2 * L
+    r = g.run(st, 6, trace_steps=steps, **kw)
+    chk = _follow_check(m, s0, r, steps, **kw)
+    assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+    if L < 4:
+        assert np.all(chk["acc"] == 1)
+
+
+def test_zero_sweeps_and_empty_batch(amh, torch, synth, gpu_model):
+    L = 16
+    g = gpu_model(L, 1000)
+    s0 = gi.initial_states(3, 2 * L, seed=2)
+    st = torch.from_numpy(s0.copy()).cuda()
+    r = g.run(st, 0)
+    assert np.array_equal(st.cpu().numpy(), s0)
+    assert np.array_equal(r["energy"].cpu().numpy(), g.energy(st).cpu().numpy())
+    assert torch.isinf(r["best_energy"]).all()
+    empty = torch.empty((0, 2 * L), dtype=torch.float32, device="cuda")
+    g.run(empty, 3)
+    assert g.energy(empty).numel() == 0
+
+
+# ---------------------------------------------------------------------------------------------
+def test_determinism_split_runs_chain_ids_and_host_entry(amh, torch, synth, gpu_model):
+    # P7 on the device
+    L, B = 32, 12
+    g = gpu_model(L, 1000)
+    s0 = gi.initial_states(B, 2 * L, seed=4)
+    kw = dict(n_global=1, n_local=3, window=6, seed=17)
+    a = torch.from_numpy(s0.copy()).cuda(); ra = g.run(a, 9, **kw)
+    b = torch.from_numpy(s0.copy()).cuda(); rb = g.run(b, 9, **kw)
+    assert torch.equal(a, b) and torch.equal(ra["energy"], rb["energy"])
+    h = torch.from_numpy(s0.copy()).cuda()
+    r1 = g.run(h, 4, **kw); r2 = g.run(h, 5, sweep_offset=4, **kw)
+    assert torch.equal(h, a)
+    assert torch.equal(torch.minimum(r1["best_energy"], r2["best_energy"]), ra["best_energy"])
+    assert torch.equal(r1["n_accept_local"] + r2["n_accept_local"], ra["n_accept_local"])
+    c = torch.from_numpy(s0[5:].copy()).cuda(); g.run(c, 9, chain_offset=5, **kw)
+    assert torch.equal(c, a[5:])
+    d = torch.from_numpy(s0.copy()).cuda(); g.run(d, 9, **dict(kw, seed=18))
+    assert not torch.equal(d, a)
+    # reported energies are the energies of the returned states
+    assert torch.allclose(ra["energy"], g.energy(a), rtol=1e-6)
+    assert torch.allclose(ra["best_energy"], g.energy(ra["best_state"]), rtol=1e-6)
+    assert (ra["best_energy"] <= ra["energy"]).all()
+    # host-buffer entry point: same trajectory
+    hs = s0.copy()
+    rh = g.run_host(hs, 9, want=("energy", "best_energy", "best_state", "n_accept_local", "n_accept_global"), **kw)
+    assert np.array_equal(hs, a.cpu().numpy())
+    assert np.array_equal(rh["energy"], ra["energy"].cpu().numpy())
+    assert np.array_equal(rh["n_accept_global"].astype(np.int64), ra["n_accept_global"].cpu().numpy())
+
+
+def test_first_hit_sweep(amh, torch, synth, gpu_model):
+    L, B = 32, 64
+    g = gpu_model(L, 1000)
+    s0 = gi.initial_states(B, 2 * L, seed=8)
+    st = torch.from_numpy(s0.copy()).cuda()
+    e0 = g.energy(st)
+    thr = float(e0.min()) * 0.9
+    r = g.run(st, 60, n_global=1, n_local=4, window=6, seed=2, energy_threshold=thr)
+    hit = int(r["first_hit_sweep"].item())
+    assert hit >= 0 and float(r["best_energy"].min()) <= thr
+    # replay sweep by sweep: the first sweep end with min energy <= thr is `hit`
+    st2 = torch.from_numpy(s0.copy()).cuda()
+    for t in range(hit + 1):
+        rr = g.run(st2, 1, sweep_offset=t, n_global=1, n_local=4, window=6, seed=2)
+        assert (float(rr["energy"].min()) <= thr) == (t == hit)
+    never = g.run(torch.from_numpy(s0.copy()).cuda(), 2, energy_threshold=-1.0)
+    assert int(never["first_hit_sweep"].item()) == -1
+
+
+def test_global_mh_boltzmann_on_device_L4(amh, orc, torch, synth, gpu_model):
+    # pin P4 run on the CUDA path: chi-square against the enumerated Boltzmann law (oracle energies)
+    from scipy import stats
+    L, G, n, T = 4, 4, 8, 1.0
+    ref, p, edges, m = synth(L, 1000)
+    g = gpu_model(L, 1000)
+    eff = [1, 2, 3, 4, 5, 6]
+    idx = np.stack(np.meshgrid(*[np.arange(G)] * 6, indexing="ij"), -1).reshape(-1, 6)
+    states = np.zeros((len(idx), n), np.float32)
+    for q, v in enumerate(eff):
+        states[:, v] = np.float32((2 * idx[:, q] - G) / np.float32(G)) * np.float32(math.pi)
+    V = m.energy(states)
+    prob = np.exp(-(V - V.min()) / T); prob /= prob.sum()
+    B = 65536
+    st = torch.from_numpy(gi.grid_states(B, n, G, seed=12)).cuda()
+    g.run(st, 40, n_global=1, n_local=0, window=0, prop_mode=amh.PROP_GRID, grid=G, seed=6, want=())
+    s = st.cpu().numpy()
+    cell = np.zeros(B, np.int64)
+    for v in eff:
+        cell = cell * G + np.rint((s[:, v].astype(np.float64) / math.pi * G + G) / 2).astype(np.int64)
+    counts = np.bincount(cell, minlength=G ** 6).astype(float)
+    expect = B * prob
+    small = expect < 5
+    cc = np.concatenate([counts[~small], [counts[small].sum()]]); ee = np.concatenate([expect[~small], [expect[small].sum()]])
+    pval = float(stats.chi2.sf(((cc - ee) ** 2 / ee).sum(), len(ee) - 1))
+    assert pval > 0.01, pval
+
+
+def test_sampled_parity_at_bench_size(amh, orc, torch, synth, gpu_model):
+    # config 1 at full width (1,024 chains, the launch shape bench.py times), a short run: energies of
+    # sampled final states against the oracle, accept counters against arithmetic bounds
+    c = gi.CONFIGS[1]
+    ref, p, edges, m = synth(c.L, c.cfg_seed)
+    g = gpu_model(c.L, c.cfg_seed)
+    st = torch.from_numpy(gi.initial_states(c.B, c.n, seed=1)).cuda()
+    r = g.run(st, 11, n_global=c.n_global, n_local=c.n_local, window=c.window, seed=1)
+    s = st.cpu().numpy()
+    rows = np.arange(0, c.B, 37)
+    want = m.energy(s[rows])
+    e = r["energy"].cpu().numpy().astype(np.float64)[rows]
+    assert np.all(np.abs(e - want) < 1e-5 * np.abs(want))
+    al, ag = r["n_accept_local"].cpu().numpy(), r["n_accept_global"].cpu().numpy()
+    assert np.all((al >= 10 * 2) & (al <= 10 * c.n)) and np.all((ag >= 2) & (ag <= c.n))
+    assert np.all(np.abs(s) <= math.pi)
+    # two rows checked step by step against the oracle over the first cycle
+    s0 = gi.initial_states(c.B, c.n, seed=1)[[0, 1023]]
+    for q, row in enumerate((0, 1023)):
+        one = torch.from_numpy(s0[q:q + 1].copy()).cuda()
+        rr = g.run(one, 2, n_global=1, n_local=10, window=8, seed=1, chain_offset=row, trace_steps=2 * c.n)
+        _follow_check(m, s0[q:q + 1], rr, 2 * c.n, n_global=1, n_local=10, window=8, seed=1, chain_offset=row)
+
+
+def test_error_codes(amh, torch, synth):
+    ref, p, edges, m = synth(8, 1000)
+    with pytest.raises(amh.AMHError) as e:
+        amh.AMH(p, np.array(list(edges[:-1]) + [100.0], np.float32))
+    assert e.value.status == 2                                   # non-uniform bins: UNSUPPORTED
+    bad = p.copy(); bad[1, 2, 3] = np.nan
+    with pytest.raises(amh.AMHError) as e:
+        amh.AMH(bad, edges)
+    assert e.value.status == 1
+    with pytest.raises(amh.AMHError) as e:
+        amh.AMH(p, edges[::-1].copy())
+    assert e.value.status == 1
+    g = amh.AMH(p, edges)
+    st = torch.from_numpy(gi.initial_states(2, 16, 1)).cuda()
+    for kw in (dict(n_global=0, n_local=0), dict(window=-1), dict(t_start=0.0, t_end=0.0), dict(prop_mode=2),
+               dict(prop_mode=1, grid=0), dict(sweep_offset=-1)):
+        with pytest.raises(amh.AMHError):
+            g.run(st, 1, **kw)
+    with pytest.raises(amh.AMHError):
+        g.energy_local(st, 16, 3)
+    # device distogram input gives the same table as the host one
+    g2 = amh.AMH(torch.from_numpy(p).cuda(), edges)
+    assert torch.equal(g.energy(st), g2.energy(st))
