@@ -244,7 +244,7 @@ def main():
         kw["per_chain_T"] = torch.from_numpy(kw["per_chain_T"]).cuda()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
     stream = torch.cuda.current_stream()
-    info = g.launch_info(B)
+    info = g.launch_info(B, cfg.window)
 
     def one_step():
         states.copy_(s0_dev)

@@ -61,6 +61,8 @@ typedef struct {
     double eps;                                  /* 1e-8, added to p inside the log */
     int    min_sep;                              /* 3: pairs need j - i >= min_sep; >= 1 */
     int    warps_per_chain;                      /* amh_run launch shape: 0 = choose from L and B; else 1,2,4,8,16 */
+    int    spec_local;                           /* local proposals evaluated per pass (one warp each, results consumed in
+                                                    order up to the first accept: same trajectory); 0 = warps_per_chain */
 } amh_options;
 
 /* Alg. 1 / Fig. 1, R10, R12. */
@@ -163,9 +165,10 @@ amh_status amh_run_host(amh_ctx *ctx, float *states, long long B, long long n_sw
 /* HOST-buffer energy: states host float [B][n] -> energy_out host float [B]; synchronises. */
 amh_status amh_energy_host(amh_ctx *ctx, const float *states, long long B, float *energy_out, void *cuda_stream);
 
-/* Launch shape amh_run would use for a batch of B rows: threads per chain-CTA, dynamic shared memory
- * bytes per CTA, CTAs resident per SM, SM count.  Any pointer may be NULL.  Host. */
-amh_status amh_launch_info(amh_ctx *ctx, long long B, int *threads_per_chain, int *smem_bytes,
+/* Launch shape amh_run would use for a batch of B rows and a schedule with this window: threads per
+ * chain-CTA, dynamic shared memory bytes per CTA, CTAs resident per SM, SM count.  Any pointer may be
+ * NULL.  Host. */
+amh_status amh_launch_info(amh_ctx *ctx, long long B, int window, int *threads_per_chain, int *smem_bytes,
                            int *ctas_per_sm, int *n_sm);
 
 /* Test hook (pin P0 on the device): out[q][0..3] = Philox4x32-10(ctr[q][0..3], key[q][0..1]).

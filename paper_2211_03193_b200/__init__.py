@@ -37,7 +37,7 @@ class AMHError(RuntimeError):
 class Options(C.Structure):
     _fields_ = [(k, C.c_double) for k in (
         "len_n_ca", "len_ca_c", "len_c_n", "ang_n_ca_c", "ang_ca_c_n", "ang_c_n_ca", "omega",
-        "cb_len", "cb_ang", "cb_dih", "eps")] + [("min_sep", C.c_int), ("warps_per_chain", C.c_int)]
+        "cb_len", "cb_ang", "cb_dih", "eps")] + [("min_sep", C.c_int), ("warps_per_chain", C.c_int), ("spec_local", C.c_int)]
 
 
 class _Schedule(C.Structure):
@@ -88,7 +88,7 @@ def lib():
                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_ulonglong, C.c_void_p, C.c_void_p]
         L.amh_run.argtypes = run_args
         L.amh_run_host.argtypes = run_args
-        L.amh_launch_info.argtypes = [C.c_void_p, C.c_longlong] + [C.POINTER(C.c_int)] * 4
+        L.amh_launch_info.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
         L.amh_philox_test.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]
         L.amh_default_options.argtypes = [C.POINTER(Options)]
         _lib = L
@@ -207,9 +207,9 @@ class AMH:
                                 _stream_ptr(stream)))
         return (cb, at) if atoms else cb
 
-    def launch_info(self, B: int) -> dict:
+    def launch_info(self, B: int, window: int = 0) -> dict:
         v = [C.c_int() for _ in range(4)]
-        _check(lib().amh_launch_info(self._h, int(B), *[C.byref(x) for x in v]))
+        _check(lib().amh_launch_info(self._h, int(B), int(window), *[C.byref(x) for x in v]))
         return dict(threads_per_chain=v[0].value, smem_bytes=v[1].value, ctas_per_sm=v[2].value, n_sm=v[3].value)
 
     # ---- amh_run ---------------------------------------------------------------------------------

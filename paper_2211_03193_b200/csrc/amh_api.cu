@@ -48,7 +48,8 @@ amh::Xf mplus(double ang, double tor, double len)
 struct amh_ctx {
     amh::DevModel m;
     amh_options opt;
-    float *E = nullptr;
+    float2 *Epk = nullptr;       // upper-triangle lerp table (see DevModel)
+    float *Elast = nullptr;
     int device = 0, n_sm = 0, max_smem = 0;
     // staging for the *_host calls (grow-only)
     void *stage = nullptr;
@@ -73,6 +74,7 @@ amh_status amh_default_options(amh_options *o)
     o->eps = 1e-8;
     o->min_sep = 3;
     o->warps_per_chain = 0;
+    o->spec_local = 0;
     return AMH_OK;
 }
 
@@ -121,6 +123,13 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.c0 = (float)(e0 + 0.5 * delta);
     m.inv_delta = (float)(1.0 / delta);
     m.tmax = (float)(n_bins - 1);
+    {
+        // smallest fp32 d^2 from which pair_energy()'s t is surely clamped to tmax: the last bin centre with a
+        // relative margin far above the rounding of sqrtf, the subtraction and the scaling (all monotone in d^2)
+        const double c_last = e0 + ((double)n_bins - 0.5) * delta;
+        const double lim = c_last * (1.0 + 1e-5) + 1e-5 * delta;
+        m.far2 = std::nextafter((float)(lim * lim), INFINITY);
+    }
     m.A = mplus(o.ang_n_ca_c, 0.0, o.len_ca_c);
     m.W = mplus(o.ang_c_n_ca, o.omega, o.len_n_ca);
     m.c2 = std::cos(o.ang_ca_c_n); m.s2 = std::sin(o.ang_ca_c_n); m.l3 = o.len_c_n;
@@ -132,11 +141,16 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.loc[3][1] = o.cb_len * std::sin(o.cb_ang) * std::cos(o.cb_dih);
     m.loc[3][2] = o.cb_len * std::sin(o.cb_ang) * std::sin(o.cb_dih);
     m.h0x = o.len_n_ca;
+    m.inv_len_n_ca = 1.0 / o.len_n_ca; m.inv_len_ca_c = 1.0 / o.len_ca_c;
 
-    if (amh::sweep_smem_bytes(n_res) > (size_t)c->max_smem) {
+    if (o.spec_local < 0 || o.spec_local > amh::kMaxWarps) {
+        delete c;
+        return fail(AMH_ERR_INVALID_ARG, "amh_create: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxWarps);
+    }
+    if (amh::sweep_smem_bytes(n_res, 0, 1) > (size_t)c->max_smem) {
         delete c;
         return fail(AMH_ERR_UNSUPPORTED, "amh_create: L = %d needs %zu B of shared memory per chain, device allows %d",
-                    n_res, amh::sweep_smem_bytes(n_res), c->max_smem);
+                    n_res, amh::sweep_smem_bytes(n_res, 0, 1), c->max_smem);
     }
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -150,7 +164,8 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     auto cleanup = [&]() {
         if (p_dev) cudaFree(p_dev);
         if (bad_dev) cudaFree(bad_dev);
-        if (c->E) cudaFree(c->E);
+        if (c->Epk) cudaFree(c->Epk);
+        if (c->Elast) cudaFree(c->Elast);
         if (c->first_hit_dev) cudaFree(c->first_hit_dev);
         delete c;
     };
@@ -163,7 +178,9 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
                         cudaGetErrorString(e_));                                                   \
         }                                                                                          \
     } while (0)
-    AMH_CUDA_C(cudaMalloc(&c->E, sizeof(float) * (size_t)count));
+    const size_t n_rows = std::max<size_t>(1, (size_t)n_res * (n_res - 1) / 2);
+    AMH_CUDA_C(cudaMalloc(&c->Epk, sizeof(float2) * n_rows * n_bins));
+    AMH_CUDA_C(cudaMalloc(&c->Elast, sizeof(float) * n_rows));
     AMH_CUDA_C(cudaMalloc(&bad_dev, sizeof(int)));
     AMH_CUDA_C(cudaMalloc(&c->first_hit_dev, sizeof(unsigned long long)));
     AMH_CUDA_C(cudaMemsetAsync(bad_dev, 0, sizeof(int), st));
@@ -176,7 +193,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     {
         const int threads = 256;
         const int blocks = (int)std::min<long long>((count + threads - 1) / threads, (long long)c->n_sm * 16);
-        amh::table_kernel<<<blocks, threads, 0, st>>>(src, c->E, count, o.eps, bad_dev);
+        amh::table_kernel<<<blocks, threads, 0, st>>>(src, c->Epk, c->Elast, n_res, n_bins, o.eps, bad_dev);
         AMH_CUDA_C(cudaGetLastError());
     }
     int bad = 0;
@@ -185,7 +202,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     if (bad) { cleanup(); return fail(AMH_ERR_INVALID_ARG, "amh_create: the distogram holds a negative, NaN or infinite value"); }
     cudaFree(bad_dev); bad_dev = nullptr;
     if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
-    m.E = c->E;
+    m.Epk = c->Epk; m.Elast = c->Elast;
     AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
     AMH_CUDA_C(cudaFuncSetAttribute(amh::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
 #undef AMH_CUDA_C
@@ -197,7 +214,8 @@ amh_status amh_destroy(amh_ctx *c)
 {
     if (!c) return AMH_OK;
     cudaDeviceSynchronize();
-    if (c->E) cudaFree(c->E);
+    if (c->Epk) cudaFree(c->Epk);
+    if (c->Elast) cudaFree(c->Elast);
     if (c->stage) cudaFree(c->stage);
     if (c->first_hit_dev) cudaFree(c->first_hit_dev);
     delete c;
@@ -249,11 +267,11 @@ amh_status amh_coords(amh_ctx *c, const float *states, long long B, float *cb_ou
 
 // warps per chain-CTA: enough lanes for the O(L^2/6) pairs of a global proposal, without starving
 // the SM of resident chains
-static int choose_warps(const amh_ctx *c, long long B)
+static int choose_warps(const amh_ctx *c, long long B, int window)
 {
     if (c->opt.warps_per_chain > 0) return c->opt.warps_per_chain;
     const int L = c->m.L;
-    const size_t smem = amh::sweep_smem_bytes(L) + 1024;
+    const size_t smem = amh::sweep_smem_bytes(L, window, 4) + 1024;
     const long long by_smem = std::max<long long>(1, (long long)(228 * 1024) / (long long)smem);
     const long long resident = std::min<long long>(B, by_smem * c->n_sm);
     const long long per_sm = std::max<long long>(1, (resident + c->n_sm - 1) / c->n_sm);
@@ -265,11 +283,11 @@ static int choose_warps(const amh_ctx *c, long long B)
     return p;
 }
 
-amh_status amh_launch_info(amh_ctx *c, long long B, int *threads_per_chain, int *smem_bytes, int *ctas_per_sm, int *n_sm)
+amh_status amh_launch_info(amh_ctx *c, long long B, int window, int *threads_per_chain, int *smem_bytes, int *ctas_per_sm, int *n_sm)
 {
     if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_launch_info: ctx is NULL");
-    const int w = choose_warps(c, std::max<long long>(B, 1));
-    const size_t smem = amh::sweep_smem_bytes(c->m.L);
+    const int w = choose_warps(c, std::max<long long>(B, 1), window);
+    const size_t smem = amh::sweep_smem_bytes(c->m.L, window, w);
     if (threads_per_chain) *threads_per_chain = 32 * w;
     if (smem_bytes) *smem_bytes = (int)smem;
     if (n_sm) *n_sm = c->n_sm;
@@ -327,8 +345,12 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
         if (a.first_hit) AMH_CUDA(cudaMemsetAsync(a.first_hit, 0xFF, sizeof(unsigned long long), st));   // -1 = none
     }
     if (B == 0) return AMH_OK;
-    const int w = choose_warps(c, B);
-    const size_t smem = amh::sweep_smem_bytes(c->m.L);
+    const int w = choose_warps(c, B, sc->window);
+    const size_t smem = amh::sweep_smem_bytes(c->m.L, sc->window, w);
+    if (smem > (size_t)c->max_smem)
+        return fail(AMH_ERR_UNSUPPORTED, "amh_run: L = %d, window = %d, %d warps need %zu B of shared memory per chain, device allows %d",
+                    c->m.L, sc->window, w, smem, c->max_smem);
+    a.spec_local = c->opt.spec_local;
     amh::sweep_kernel<<<(unsigned)B, 32 * w, smem, st>>>(c->m, a);
     AMH_CUDA(cudaGetLastError());
     return AMH_OK;

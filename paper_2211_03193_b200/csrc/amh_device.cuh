@@ -22,14 +22,20 @@ struct Xf {            // x -> R x + t, R row-major
 
 struct DevModel {
     int L, nb, min_sep, n;           // residues, bins, minimum sequence separation, variables (2L)
-    const float *E;                  // [L][L][nb]  E = -log(p + eps)
+    // Energy table, upper triangle only (R9: only p[i][j], i < j, is read).  Row r = tri(i, j) of pair i < j:
+    //   Epk[r][b]   = { E[b], E[min(b+1, nb-1)] - E[b] },  E = -log(p + eps)   (the two operands of R8's lerp)
+    //   Elast[r]    = e_ij(d) for every d >= the last bin centre (the clamped value of R8)
+    const float2 *Epk;
+    const float *Elast;
     float c0, inv_delta, tmax;       // first bin centre, 1/bin width, nb-1
+    float far2;                      // d^2 >= far2  =>  the clamp of R8 applies: e_ij(d) = Elast
     // bond-frame recursion H_{i+1} = H_i * A * Mplus(theta2, psi_i) * W * Rx(phi_{i+1})
     Xf A;                            // place C_i from the N->CA bond frame: Mplus(ang_n_ca_c, 0, len_ca_c)
     Xf W;                            // Mplus(ang_c_n_ca, omega, len_n_ca)
     double c2, s2, l3;               // cos/sin of ang_ca_c_n, len_c_n
     double loc[4][3];                // N, CA, C, CB in the residue's bond frame (origin CA, x along N->CA)
     double h0x;                      // H_0 = [I | (len_n_ca, 0, 0)]
+    double inv_len_n_ca, inv_len_ca_c;   // 1 / length of the bonds the torsions turn about
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -171,7 +177,7 @@ __device__ __forceinline__ void nerf_build_warp(const DevModel &m, const float *
 // Pair term (Eq. 3a, R8): linear interpolation of E between bin centres, clamped at the end centres.
 // d2 = 0 is safe (IEEE sqrt), so coincident atoms score E[0].
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ float pair_energy(const float *__restrict__ row, float d2, float c0, float inv_delta, float tmax, int nb)
+__device__ __forceinline__ float pair_energy(const float2 *__restrict__ row, float d2, float c0, float inv_delta, float tmax, int nb)
 {
     const float d = sqrtf(d2);
     float t = (d - c0) * inv_delta;
@@ -179,8 +185,14 @@ __device__ __forceinline__ float pair_energy(const float *__restrict__ row, floa
     int b = (int)t;
     b = min(b, nb - 2);
     const float f = t - (float)b;
-    const float e0 = __ldg(row + b), e1 = __ldg(row + b + 1);
-    return fmaf(f, e1 - e0, e0);
+    const float2 v = __ldg(row + b);              // { E[b], E[b+1] - E[b] }: one 8-byte gather per evaluation
+    return fmaf(f, v.y, v.x);
+}
+
+// row index of the pair i < j in the upper-triangle tables: tri(i, j) = tri_base(i) + j
+__device__ __forceinline__ long long tri_base(int i, int L)
+{
+    return (long long)i * (2 * L - i - 1) / 2 - i - 1;
 }
 
 __device__ __forceinline__ double warp_sum(double v)

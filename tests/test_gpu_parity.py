@@ -153,11 +153,13 @@ def _follow_check(m, s0, r, steps, **kw):
     return dict(err=err, n_diff=int(diff.sum()), n_near=int(near.sum()), f=f, acc=acc)
 
 
-@pytest.mark.parametrize("wpc", [0, 1, 4])
-def test_trajectory_parity_config0_first_1000_steps(amh, orc, torch, synth, wpc):
+@pytest.mark.parametrize("wpc,spec", [(0, 0), (1, 0), (4, 0), (4, 1), (8, 3), (16, 0)])
+def test_trajectory_parity_config0_first_1000_steps(amh, orc, torch, synth, wpc, spec):
+    # every launch shape walks the same trajectory: warps per chain, and how many local proposals are
+    # evaluated per pass (spec = 1 is the plain sequential order of Alg. 1)
     c = gi.CONFIGS[0]
     ref, p, edges, m = synth(c.L, c.cfg_seed)
-    g = amh.AMH(p, edges, amh.default_options(warps_per_chain=wpc))
+    g = amh.AMH(p, edges, amh.default_options(warps_per_chain=wpc, spec_local=spec))
     s0 = gi.initial_states(c.B, c.n, seed=1)
     st = torch.from_numpy(s0.copy()).cuda()
     steps = 1024                           # 8 full sweeps: steps 0..999 are the bar (R21), 24 more close the sweep
@@ -165,8 +167,8 @@ def test_trajectory_parity_config0_first_1000_steps(amh, orc, torch, synth, wpc)
     r = g.run(st, 8, trace_steps=steps, **kw)
     chk = _follow_check(m, s0, r, steps, **kw)
     err = chk["err"]
-    print("cfg0 wpc=%d: |dE_gpu - dE_oracle| median %.2e  p99 %.2e  max %.2e; decisions differing %d, near-ties %d of %d"
-          % (wpc, np.median(err), np.quantile(err, 0.99), err.max(), chk["n_diff"], chk["n_near"], err.size))
+    print("cfg0 wpc=%d spec=%d: |dE_gpu - dE_oracle| median %.2e  p99 %.2e  max %.2e; decisions differing %d, near-ties %d of %d"
+          % (wpc, spec, np.median(err), np.quantile(err, 0.99), err.max(), chk["n_diff"], chk["n_near"], err.size))
     assert err.max() < 2e-3
     assert np.quantile(err, 0.99) < 3e-4
     # first 1000 steps = 128 global + 872 local proposals: both phases are exercised
