@@ -176,6 +176,9 @@ def main():
     ap.add_argument("--sweeps", type=int, default=0, help="override the config's sweep count (experiments only; the line says so)")
     ap.add_argument("--chains", type=int, default=0, help="override the config's chain count (experiments only)")
     ap.add_argument("--warps-per-chain", type=int, default=0)
+    ap.add_argument("--chains-per-cta", type=int, default=0)
+    ap.add_argument("--spec-local", type=int, default=0)
+    ap.add_argument("--ring-cols", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -233,7 +236,8 @@ def main():
     g0.close()
     D = np.linalg.norm(cb[:, None] - cb[None], axis=-1)
     p = gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi)
-    g = pkg.AMH(p, edges, pkg.default_options(warps_per_chain=args.warps_per_chain))
+    g = pkg.AMH(p, edges, pkg.default_options(warps_per_chain=args.warps_per_chain, chains_per_cta=args.chains_per_cta,
+                                               spec_local=args.spec_local, ring_cols=args.ring_cols))
     del p
     chain_offset = rank * B
     s0_host = torch.from_numpy(gi.initial_states(B, n, seed=1, chain_offset=chain_offset)).pin_memory()
@@ -322,7 +326,8 @@ def main():
         cpu_baseline, _ = oracle_leg(cfg, min(cfg.B, 64), min(cfg.n_sweeps, 2 * (cfg.n_global + cfg.n_local)))
 
     workload.update(l2="flushed between timed steps (256 MiB write)", threads_per_chain=info["threads_per_chain"],
-                    smem_bytes_per_chain=info["smem_bytes"], chains_resident_per_sm=info["ctas_per_sm"],
+                    chains_per_cta=info["chains_per_cta"], ring_cols=info["ring_cols"], ring_rows=info["ring_rows"],
+                    smem_bytes_per_cta=info["smem_bytes"], ctas_resident_per_sm=info["ctas_per_sm"],
                     step="amh_run over the full config from the seeded random start", best_energy=best)
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",

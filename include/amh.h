@@ -60,9 +60,13 @@ typedef struct {
     double cb_len, cb_ang, cb_dih;               /* |CA-CB| 1.522, angle N-CA-CB 1.927, dihedral C-N-CA-CB -2.143 */
     double eps;                                  /* 1e-8, added to p inside the log */
     int    min_sep;                              /* 3: pairs need j - i >= min_sep; >= 1 */
-    int    warps_per_chain;                      /* amh_run launch shape: 0 = choose from L and B; else 1,2,4,8,16 */
+    int    warps_per_chain;                      /* amh_run launch shape: 0 = choose from L and B; else 1..15 */
     int    spec_local;                           /* local proposals evaluated per pass (one warp each, results consumed in
                                                     order up to the first accept: same trajectory); 0 = warps_per_chain */
+    int    chains_per_cta;                       /* chains sharing one CTA and its table ring: 0 = choose; else 1..15,
+                                                    chains_per_cta * warps_per_chain <= 15 */
+    int    ring_cols;                            /* slots of the shared-memory table ring of the local phase: 0 = choose,
+                                                    -1 = off (rows gathered from L2), else >= window + 3 */
 } amh_options;
 
 /* Alg. 1 / Fig. 1, R10, R12. */
@@ -170,6 +174,11 @@ amh_status amh_energy_host(amh_ctx *ctx, const float *states, long long B, float
  * NULL.  Host. */
 amh_status amh_launch_info(amh_ctx *ctx, long long B, int window, int *threads_per_chain, int *smem_bytes,
                            int *ctas_per_sm, int *n_sm);
+
+/* The rest of the launch shape: chains per CTA, warps per chain, slots and rows per slot of the table
+ * ring (0, 0 = ring off).  Any pointer may be NULL.  Host. */
+amh_status amh_launch_shape(amh_ctx *ctx, long long B, int window, int *chains_per_cta, int *warps_per_chain,
+                            int *ring_cols, int *ring_rows);
 
 /* Test hook (pin P0 on the device): out[q][0..3] = Philox4x32-10(ctr[q][0..3], key[q][0..1]).
  * ctr: DEVICE uint32 [count][4]; key: DEVICE uint32 [count][2]; out: DEVICE uint32 [count][4]. */

@@ -24,7 +24,7 @@ PROP_UNIFORM, PROP_GRID = 0, 1
 
 # every symbol include/amh.h declares
 EXPORTS = ["amh_default_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
-           "amh_run", "amh_run_host", "amh_energy_host", "amh_launch_info", "amh_philox_test",
+           "amh_run", "amh_run_host", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
            "amh_last_error", "amh_version"]
 
 
@@ -37,7 +37,8 @@ class AMHError(RuntimeError):
 class Options(C.Structure):
     _fields_ = [(k, C.c_double) for k in (
         "len_n_ca", "len_ca_c", "len_c_n", "ang_n_ca_c", "ang_ca_c_n", "ang_c_n_ca", "omega",
-        "cb_len", "cb_ang", "cb_dih", "eps")] + [("min_sep", C.c_int), ("warps_per_chain", C.c_int), ("spec_local", C.c_int)]
+        "cb_len", "cb_ang", "cb_dih", "eps")] + [("min_sep", C.c_int), ("warps_per_chain", C.c_int), ("spec_local", C.c_int),
+                                         ("chains_per_cta", C.c_int), ("ring_cols", C.c_int)]
 
 
 class _Schedule(C.Structure):
@@ -89,6 +90,7 @@ def lib():
         L.amh_run.argtypes = run_args
         L.amh_run_host.argtypes = run_args
         L.amh_launch_info.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
+        L.amh_launch_shape.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
         L.amh_philox_test.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]
         L.amh_default_options.argtypes = [C.POINTER(Options)]
         _lib = L
@@ -210,7 +212,10 @@ class AMH:
     def launch_info(self, B: int, window: int = 0) -> dict:
         v = [C.c_int() for _ in range(4)]
         _check(lib().amh_launch_info(self._h, int(B), int(window), *[C.byref(x) for x in v]))
-        return dict(threads_per_chain=v[0].value, smem_bytes=v[1].value, ctas_per_sm=v[2].value, n_sm=v[3].value)
+        u = [C.c_int() for _ in range(4)]
+        _check(lib().amh_launch_shape(self._h, int(B), int(window), *[C.byref(x) for x in u]))
+        return dict(threads_per_chain=v[0].value, smem_bytes=v[1].value, ctas_per_sm=v[2].value, n_sm=v[3].value,
+                    chains_per_cta=u[0].value, warps_per_chain=u[1].value, ring_cols=u[2].value, ring_rows=u[3].value)
 
     # ---- amh_run ---------------------------------------------------------------------------------
     @staticmethod

@@ -9,6 +9,7 @@
 
 #include "../../include/amh.h"
 #include "amh_kernels.cuh"
+#include "amh_sweep.cuh"
 
 namespace {
 
@@ -50,6 +51,7 @@ struct amh_ctx {
     amh_options opt;
     float2 *Epk = nullptr;       // upper-triangle lerp table (see DevModel)
     float *Elast = nullptr;
+    float *Epl = nullptr;        // the same E, plain rows padded to row_stride floats (TMA source)
     int device = 0, n_sm = 0, max_smem = 0;
     // staging for the *_host calls (grow-only)
     void *stage = nullptr;
@@ -75,6 +77,8 @@ amh_status amh_default_options(amh_options *o)
     o->min_sep = 3;
     o->warps_per_chain = 0;
     o->spec_local = 0;
+    o->chains_per_cta = 0;
+    o->ring_cols = 0;
     return AMH_OK;
 }
 
@@ -95,8 +99,13 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     if (!(o.eps >= 0.0)) return fail(AMH_ERR_INVALID_ARG, "amh_create: eps < 0");
     {
         const int w = o.warps_per_chain;
-        if (!(w == 0 || w == 1 || w == 2 || w == 4 || w == 8 || w == 16))
-            return fail(AMH_ERR_INVALID_ARG, "amh_create: warps_per_chain = %d not in {0,1,2,4,8,16}", w);
+        if (w < 0 || w > amh::kMaxTeamWarps)
+            return fail(AMH_ERR_INVALID_ARG, "amh_create: warps_per_chain = %d outside [0, %d]", w, amh::kMaxTeamWarps);
+        const int cc = o.chains_per_cta;
+        if (cc < 0 || cc > amh::kMaxChains)
+            return fail(AMH_ERR_INVALID_ARG, "amh_create: chains_per_cta = %d outside [0, %d]", cc, amh::kMaxChains);
+        if (w > 0 && cc > 0 && w * cc > amh::kMaxTeamWarps)
+            return fail(AMH_ERR_INVALID_ARG, "amh_create: warps_per_chain * chains_per_cta = %d > %d", w * cc, amh::kMaxTeamWarps);
     }
     for (int b = 0; b <= n_bins; ++b)
         if (!std::isfinite(bin_edges[b])) return fail(AMH_ERR_INVALID_ARG, "amh_create: bin edge %d is not finite", b);
@@ -143,14 +152,14 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.h0x = o.len_n_ca;
     m.inv_len_n_ca = 1.0 / o.len_n_ca; m.inv_len_ca_c = 1.0 / o.len_ca_c;
 
-    if (o.spec_local < 0 || o.spec_local > amh::kMaxWarps) {
+    if (o.spec_local < 0 || o.spec_local > amh::kMaxTeamWarps) {
         delete c;
-        return fail(AMH_ERR_INVALID_ARG, "amh_create: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxWarps);
+        return fail(AMH_ERR_INVALID_ARG, "amh_create: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxTeamWarps);
     }
-    if (amh::sweep_smem_bytes(n_res, 0, 1) > (size_t)c->max_smem) {
+    if (amh::sweep_smem_bytes(n_res, 0, 1, 1, 0, 0, 0) > (size_t)c->max_smem) {
         delete c;
         return fail(AMH_ERR_UNSUPPORTED, "amh_create: L = %d needs %zu B of shared memory per chain, device allows %d",
-                    n_res, amh::sweep_smem_bytes(n_res, 0, 1), c->max_smem);
+                    n_res, amh::sweep_smem_bytes(n_res, 0, 1, 1, 0, 0, 0), c->max_smem);
     }
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -166,6 +175,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
         if (bad_dev) cudaFree(bad_dev);
         if (c->Epk) cudaFree(c->Epk);
         if (c->Elast) cudaFree(c->Elast);
+        if (c->Epl) cudaFree(c->Epl);
         if (c->first_hit_dev) cudaFree(c->first_hit_dev);
         delete c;
     };
@@ -181,6 +191,13 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     const size_t n_rows = std::max<size_t>(1, (size_t)n_res * (n_res - 1) / 2);
     AMH_CUDA_C(cudaMalloc(&c->Epk, sizeof(float2) * n_rows * n_bins));
     AMH_CUDA_C(cudaMalloc(&c->Elast, sizeof(float) * n_rows));
+    {
+        int stride = (n_bins + 3) & ~3;
+        while ((stride & 7) != 4) stride += 4;          // 16-byte multiple, bank offset 4 (mod 8) words per row
+        m.row_stride = stride;
+    }
+    AMH_CUDA_C(cudaMalloc(&c->Epl, sizeof(float) * n_rows * m.row_stride));
+    AMH_CUDA_C(cudaMemsetAsync(c->Epl, 0, sizeof(float) * n_rows * m.row_stride, st));
     AMH_CUDA_C(cudaMalloc(&bad_dev, sizeof(int)));
     AMH_CUDA_C(cudaMalloc(&c->first_hit_dev, sizeof(unsigned long long)));
     AMH_CUDA_C(cudaMemsetAsync(bad_dev, 0, sizeof(int), st));
@@ -193,7 +210,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     {
         const int threads = 256;
         const int blocks = (int)std::min<long long>((count + threads - 1) / threads, (long long)c->n_sm * 16);
-        amh::table_kernel<<<blocks, threads, 0, st>>>(src, c->Epk, c->Elast, n_res, n_bins, o.eps, bad_dev);
+        amh::table_kernel<<<blocks, threads, 0, st>>>(src, c->Epk, c->Elast, c->Epl, m.row_stride, n_res, n_bins, o.eps, bad_dev);
         AMH_CUDA_C(cudaGetLastError());
     }
     int bad = 0;
@@ -202,7 +219,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     if (bad) { cleanup(); return fail(AMH_ERR_INVALID_ARG, "amh_create: the distogram holds a negative, NaN or infinite value"); }
     cudaFree(bad_dev); bad_dev = nullptr;
     if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
-    m.Epk = c->Epk; m.Elast = c->Elast;
+    m.Epk = c->Epk; m.Elast = c->Elast; m.Epl = c->Epl;
     AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
     AMH_CUDA_C(cudaFuncSetAttribute(amh::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
 #undef AMH_CUDA_C
@@ -216,6 +233,7 @@ amh_status amh_destroy(amh_ctx *c)
     cudaDeviceSynchronize();
     if (c->Epk) cudaFree(c->Epk);
     if (c->Elast) cudaFree(c->Elast);
+    if (c->Epl) cudaFree(c->Epl);
     if (c->stage) cudaFree(c->stage);
     if (c->first_hit_dev) cudaFree(c->first_hit_dev);
     delete c;
@@ -265,37 +283,67 @@ amh_status amh_coords(amh_ctx *c, const float *states, long long B, float *cb_ou
     return AMH_OK;
 }
 
-// warps per chain-CTA: enough lanes for the O(L^2/6) pairs of a global proposal, without starving
-// the SM of resident chains
-static int choose_warps(const amh_ctx *c, long long B, int window)
+// Launch shape of amh_run: C chains per CTA, W warps per chain, R ring slots.
+struct SweepShape { int C, W, R, ring_rows; size_t smem; };
+
+static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
 {
-    if (c->opt.warps_per_chain > 0) return c->opt.warps_per_chain;
     const int L = c->m.L;
-    const size_t smem = amh::sweep_smem_bytes(L, window, 4) + 1024;
-    const long long by_smem = std::max<long long>(1, (long long)(228 * 1024) / (long long)smem);
-    const long long resident = std::min<long long>(B, by_smem * c->n_sm);
-    const long long per_sm = std::max<long long>(1, (resident + c->n_sm - 1) / c->n_sm);
-    const long long by_occ = std::max<long long>(1, 48 / per_sm);
-    const long long by_work = std::max<long long>(1, ((long long)L * L / 6) / (32 * 8));
-    long long w = std::min(by_occ, by_work);
-    int p = 1;
-    while (2 * p <= w && p < 16) p *= 2;
-    return p;
+    const int w_eff = std::min(window, std::max(L - 1, 0));
+    const int span = std::min(2 * window, std::max(L - 1, 0));
+    SweepShape sh;
+    sh.ring_rows = std::max(0, span - c->m.min_sep + 1);
+    const size_t budget = (size_t)c->max_smem;
+    auto ring_for = [&](int C) -> int {                       // slots: the window's columns + prefetch + drift between teams
+        if (c->opt.ring_cols < 0 || sh.ring_rows == 0) return 0;
+        if (c->opt.ring_cols > 0) return std::max(c->opt.ring_cols, w_eff + 3);
+        return w_eff + 3 + (C > 1 ? 6 : 2);
+    };
+    auto fits = [&](int C, int W, int R) { return amh::sweep_smem_bytes(L, window, C, W, R, sh.ring_rows, c->m.row_stride) <= budget; };
+    // chains per CTA: spread the batch over the SMs, one CTA each
+    int C = c->opt.chains_per_cta;
+    if (C <= 0) C = (int)std::min<long long>(8, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));
+    int W = c->opt.warps_per_chain;
+    auto auto_w = [&](int C_) { return std::max(1, std::min(amh::kMaxTeamWarps / C_, 8)); };
+    int R;
+    for (;;) {
+        const int Wc = W > 0 ? std::max(1, std::min(W, amh::kMaxTeamWarps / C)) : auto_w(C);
+        R = ring_for(C);
+        if (fits(C, Wc, R)) { W = Wc; break; }
+        if (c->opt.chains_per_cta <= 0 && C > 1) { --C; continue; }
+        R = 0;                                               // the ring does not fit: rows are gathered from L2
+        W = Wc;
+        break;
+    }
+    sh.C = C; sh.W = W; sh.R = R;
+    if (R == 0) sh.ring_rows = 0;
+    sh.smem = amh::sweep_smem_bytes(L, window, C, W, R, sh.ring_rows, c->m.row_stride);
+    return sh;
 }
 
 amh_status amh_launch_info(amh_ctx *c, long long B, int window, int *threads_per_chain, int *smem_bytes, int *ctas_per_sm, int *n_sm)
 {
     if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_launch_info: ctx is NULL");
-    const int w = choose_warps(c, std::max<long long>(B, 1), window);
-    const size_t smem = amh::sweep_smem_bytes(c->m.L, window, w);
-    if (threads_per_chain) *threads_per_chain = 32 * w;
-    if (smem_bytes) *smem_bytes = (int)smem;
+    const SweepShape sh = choose_shape(c, std::max<long long>(B, 1), window);
+    if (threads_per_chain) *threads_per_chain = 32 * sh.W;
+    if (smem_bytes) *smem_bytes = (int)sh.smem;
     if (n_sm) *n_sm = c->n_sm;
     if (ctas_per_sm) {
         int nb = 0;
-        AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::sweep_kernel, 32 * w, smem));
+        AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::sweep_kernel, 32 * (sh.C * sh.W + 1), sh.smem));
         *ctas_per_sm = nb;
     }
+    return AMH_OK;
+}
+
+amh_status amh_launch_shape(amh_ctx *c, long long B, int window, int *chains_per_cta, int *warps_per_chain, int *ring_cols, int *ring_rows)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_launch_shape: ctx is NULL");
+    const SweepShape sh = choose_shape(c, std::max<long long>(B, 1), window);
+    if (chains_per_cta) *chains_per_cta = sh.C;
+    if (warps_per_chain) *warps_per_chain = sh.W;
+    if (ring_cols) *ring_cols = sh.R;
+    if (ring_rows) *ring_rows = sh.ring_rows;
     return AMH_OK;
 }
 
@@ -345,13 +393,14 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
         if (a.first_hit) AMH_CUDA(cudaMemsetAsync(a.first_hit, 0xFF, sizeof(unsigned long long), st));   // -1 = none
     }
     if (B == 0) return AMH_OK;
-    const int w = choose_warps(c, B, sc->window);
-    const size_t smem = amh::sweep_smem_bytes(c->m.L, sc->window, w);
-    if (smem > (size_t)c->max_smem)
-        return fail(AMH_ERR_UNSUPPORTED, "amh_run: L = %d, window = %d, %d warps need %zu B of shared memory per chain, device allows %d",
-                    c->m.L, sc->window, w, smem, c->max_smem);
+    const SweepShape sh = choose_shape(c, B, sc->window);
+    if (sh.smem > (size_t)c->max_smem)
+        return fail(AMH_ERR_UNSUPPORTED, "amh_run: L = %d, window = %d, %d chains x %d warps need %zu B of shared memory, device allows %d",
+                    c->m.L, sc->window, sh.C, sh.W, sh.smem, c->max_smem);
+    a.C = sh.C; a.W = sh.W; a.ring_cols = sh.R; a.ring_rows = sh.ring_rows;
     a.spec_local = c->opt.spec_local;
-    amh::sweep_kernel<<<(unsigned)B, 32 * w, smem, st>>>(c->m, a);
+    const long long ctas = (B + sh.C - 1) / sh.C;
+    amh::sweep_kernel<<<(unsigned)ctas, 32 * (sh.C * sh.W + 1), sh.smem, st>>>(c->m, a);
     AMH_CUDA(cudaGetLastError());
     return AMH_OK;
 }

@@ -25,8 +25,12 @@ struct DevModel {
     // Energy table, upper triangle only (R9: only p[i][j], i < j, is read).  Row r = tri(i, j) of pair i < j:
     //   Epk[r][b]   = { E[b], E[min(b+1, nb-1)] - E[b] },  E = -log(p + eps)   (the two operands of R8's lerp)
     //   Elast[r]    = e_ij(d) for every d >= the last bin centre (the clamped value of R8)
+    //   Epl[r][b]   = E[b], rows padded to row_stride floats (16-byte multiples whose bank offset differs from row
+    //                 to row): what the TMA bulk copies stage into shared memory for the local phase
     const float2 *Epk;
     const float *Elast;
+    const float *Epl;
+    int row_stride;
     float c0, inv_delta, tmax;       // first bin centre, 1/bin width, nb-1
     float far2;                      // d^2 >= far2  =>  the clamp of R8 applies: e_ij(d) = Elast
     // bond-frame recursion H_{i+1} = H_i * A * Mplus(theta2, psi_i) * W * Rx(phi_{i+1})
