@@ -179,6 +179,7 @@ def main():
     ap.add_argument("--chains-per-cta", type=int, default=0)
     ap.add_argument("--spec-local", type=int, default=0)
     ap.add_argument("--ring-cols", type=int, default=0)
+    ap.add_argument("--lanes-per-step", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -237,7 +238,8 @@ def main():
     D = np.linalg.norm(cb[:, None] - cb[None], axis=-1)
     p = gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi)
     g = pkg.AMH(p, edges, pkg.default_options(warps_per_chain=args.warps_per_chain, chains_per_cta=args.chains_per_cta,
-                                               spec_local=args.spec_local, ring_cols=args.ring_cols))
+                                               spec_local=args.spec_local, ring_cols=args.ring_cols,
+                                               lanes_per_step=args.lanes_per_step))
     del p
     chain_offset = rank * B
     s0_host = torch.from_numpy(gi.initial_states(B, n, seed=1, chain_offset=chain_offset)).pin_memory()

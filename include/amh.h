@@ -61,8 +61,10 @@ typedef struct {
     double eps;                                  /* 1e-8, added to p inside the log */
     int    min_sep;                              /* 3: pairs need j - i >= min_sep; >= 1 */
     int    warps_per_chain;                      /* amh_run launch shape: 0 = choose from L and B; else 1..15 */
-    int    spec_local;                           /* local proposals evaluated per pass (one warp each, results consumed in
-                                                    order up to the first accept: same trajectory); 0 = warps_per_chain */
+    int    spec_local;                           /* local proposals evaluated per pass (results consumed in order up to the
+                                                    first accept: same trajectory); 0 = as many as the team has lane groups,
+                                                    at most 16 */
+    int    lanes_per_step;                       /* lanes that share one local proposal: 0 = choose; else 8, 16 or 32 */
     int    chains_per_cta;                       /* chains sharing one CTA and its table ring: 0 = choose; else 1..15,
                                                     chains_per_cta * warps_per_chain <= 15 */
     int    ring_cols;                            /* slots of the shared-memory table ring of the local phase: 0 = choose,

@@ -79,6 +79,7 @@ amh_status amh_default_options(amh_options *o)
     o->spec_local = 0;
     o->chains_per_cta = 0;
     o->ring_cols = 0;
+    o->lanes_per_step = 0;
     return AMH_OK;
 }
 
@@ -152,14 +153,18 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.h0x = o.len_n_ca;
     m.inv_len_n_ca = 1.0 / o.len_n_ca; m.inv_len_ca_c = 1.0 / o.len_ca_c;
 
-    if (o.spec_local < 0 || o.spec_local > amh::kMaxTeamWarps) {
+    if (!(o.lanes_per_step == 0 || o.lanes_per_step == 8 || o.lanes_per_step == 16 || o.lanes_per_step == 32)) {
         delete c;
-        return fail(AMH_ERR_INVALID_ARG, "amh_create: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxTeamWarps);
+        return fail(AMH_ERR_INVALID_ARG, "amh_create: lanes_per_step = %d not in {0, 8, 16, 32}", o.lanes_per_step);
     }
-    if (amh::sweep_smem_bytes(n_res, 0, 1, 1, 0, 0, 0) > (size_t)c->max_smem) {
+    if (o.spec_local < 0 || o.spec_local > amh::kMaxSpec) {
+        delete c;
+        return fail(AMH_ERR_INVALID_ARG, "amh_create: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxSpec);
+    }
+    if (amh::sweep_smem_bytes(n_res, 1, 0, 0, 0) > (size_t)c->max_smem) {
         delete c;
         return fail(AMH_ERR_UNSUPPORTED, "amh_create: L = %d needs %zu B of shared memory per chain, device allows %d",
-                    n_res, amh::sweep_smem_bytes(n_res, 0, 1, 1, 0, 0, 0), c->max_smem);
+                    n_res, amh::sweep_smem_bytes(n_res, 1, 0, 0, 0), c->max_smem);
     }
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -297,9 +302,9 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
     auto ring_for = [&](int C) -> int {                       // slots: the window's columns + prefetch + drift between teams
         if (c->opt.ring_cols < 0 || sh.ring_rows == 0) return 0;
         if (c->opt.ring_cols > 0) return std::max(c->opt.ring_cols, w_eff + 3);
-        return w_eff + 3 + (C > 1 ? 6 : 2);
+        return w_eff + 3 + amh::kMaxSpec / 2 + (C > 1 ? 4 : 0);    // + reach of a speculative pass + drift between teams
     };
-    auto fits = [&](int C, int W, int R) { return amh::sweep_smem_bytes(L, window, C, W, R, sh.ring_rows, c->m.row_stride) <= budget; };
+    auto fits = [&](int C, int, int R) { return amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride) <= budget; };
     // chains per CTA: spread the batch over the SMs, one CTA each
     int C = c->opt.chains_per_cta;
     if (C <= 0) C = (int)std::min<long long>(8, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));
@@ -317,7 +322,7 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
     }
     sh.C = C; sh.W = W; sh.R = R;
     if (R == 0) sh.ring_rows = 0;
-    sh.smem = amh::sweep_smem_bytes(L, window, C, W, R, sh.ring_rows, c->m.row_stride);
+    sh.smem = amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride);
     return sh;
 }
 
@@ -399,6 +404,7 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
                     c->m.L, sc->window, sh.C, sh.W, sh.smem, c->max_smem);
     a.C = sh.C; a.W = sh.W; a.ring_cols = sh.R; a.ring_rows = sh.ring_rows;
     a.spec_local = c->opt.spec_local;
+    a.lanes_per_step = c->opt.lanes_per_step > 0 ? c->opt.lanes_per_step : 16;
     const long long ctas = (B + sh.C - 1) / sh.C;
     amh::sweep_kernel<<<(unsigned)ctas, 32 * (sh.C * sh.W + 1), sh.smem, st>>>(c->m, a);
     AMH_CUDA(cudaGetLastError());

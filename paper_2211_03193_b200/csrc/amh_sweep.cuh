@@ -35,7 +35,8 @@ struct RunArgs {
     int prop_mode, grid;
     // launch shape
     int C, W;                            // chains per CTA, warps per chain
-    int spec_local;                      // local proposals evaluated per pass (<= W)
+    int spec_local;                      // local proposals evaluated per pass (<= W * 32 / lanes_per_step, <= 16)
+    int lanes_per_step;                  // lanes that share one local proposal: 32, 16 or 8
     int ring_cols;                       // R: slots of the table ring (> window + 2), 0 = gather from L2 instead
     int ring_rows;                       // rows per column: 2w - min_sep + 1
     unsigned long long seed;
@@ -49,19 +50,22 @@ struct RunArgs {
     unsigned char *trace_acc;
 };
 
-constexpr int kDrawBatch = 32;           // steps whose draws are generated together, one lane per step
+constexpr int kDrawBatch = 64;           // steps whose draws are generated together, two per lane
 constexpr int kMaxWarps = 16;            // array bound of the per-warp scratch of a team
+constexpr int kMaxSpec = 16;             // local proposals evaluated per pass, at most
 constexpr int kMaxTeamWarps = 15;        // team warps per CTA: chains x warps per chain (+ the producer = 512 threads)
 constexpr int kMaxChains = 15;           // chains per CTA (named barriers 1..15)
 constexpr int kSweepMaxThreads = 512;    // 15 team warps + the producer: 128 registers per thread
 
-__host__ __device__ inline int sweep_wcap(int L, int window) { return (window + 1 < L) ? window + 1 : L; }
-
-// shared memory of one chain, in bytes (a multiple of 16)
-__host__ __device__ inline size_t chain_smem_bytes(int L, int window, int W)
+// shared memory of one chain, in bytes (a multiple of 16):
+//   double X[4L], Y[4L], Z[4L]   atoms, index atom * L + res (atom 0..3 = N, CA, C, CB)
+//   double red[16], b_cd[64], b_sd[64], b_lu[64], rot_s[16][12], sp_dE[16]
+//   float4 cb4[L]                fp32 copy of the C-betas (what the pair loops read)
+//   float  s[n], b_sp[64];  int sp_acc[16]
+__host__ __device__ inline size_t chain_smem_bytes(int L)
 {
-    const size_t doubles = 12 * (size_t)L + kMaxWarps + 3 * kDrawBatch + 12 * kMaxWarps + kMaxWarps;
-    size_t floats = 6 * (size_t)L + 2 * (size_t)L + kDrawBatch + (size_t)W * 3 * sweep_wcap(L, window) + kMaxWarps;
+    const size_t doubles = 12 * (size_t)L + kMaxWarps + 3 * kDrawBatch + 12 * kMaxSpec + kMaxSpec;
+    size_t floats = 4 * (size_t)L + 2 * (size_t)L + kDrawBatch + kMaxSpec;
     floats = (floats + 3) & ~(size_t)3;
     return sizeof(double) * doubles + sizeof(float) * floats;
 }
@@ -69,11 +73,11 @@ __host__ __device__ inline size_t chain_smem_bytes(int L, int window, int W)
 // header: ring barriers, progress words; then the ring; then the chains
 __host__ __device__ inline size_t sweep_header_bytes(int ring_cols) { return (8 * (size_t)ring_cols + 8 * 16 + 15) & ~(size_t)15; }
 
-__host__ __device__ inline size_t sweep_smem_bytes(int L, int window, int C, int W, int ring_cols, int ring_rows, int row_stride)
+__host__ __device__ inline size_t sweep_smem_bytes(int L, int C, int ring_cols, int ring_rows, int row_stride)
 {
     size_t b = sweep_header_bytes(ring_cols) + sizeof(float) * (size_t)ring_cols * ring_rows * row_stride;
     b = (b + 15) & ~(size_t)15;
-    return b + (size_t)C * chain_smem_bytes(L, window, W);
+    return b + (size_t)C * chain_smem_bytes(L);
 }
 
 // ---- PTX: mbarrier, TMA bulk copy, named barriers ----------------------------------------------------
@@ -155,6 +159,23 @@ __device__ __forceinline__ float pair_energy_row(const float *row, float d2, flo
     return fmaf(f, e1 - e0, e0);
 }
 
+
+// bin index and fraction of R8's interpolation at squared distance d2.  d = sqrt(d2) by one reciprocal-square-root
+// and one Newton step: within 1 ulp of the correctly rounded root (the coordinates feeding d2
+// are themselves rounded to fp32), at 5 instructions instead of sqrtf()'s 9 with its special-case branch.  d2 = 0
+// (coincident atoms) is mapped to the first bin by the floor below.
+__device__ __forceinline__ void lerp_coords(float d2, float c0, float inv_delta, float tmax, int nb, int &b, float &f)
+{
+    d2 = fmaxf(d2, 1e-30f);
+    const float r = rsqrtf(d2);
+    float d = d2 * r;
+    d = fmaf(0.5f * r, fmaf(-d, d, d2), d);
+    float t = (d - c0) * inv_delta;
+    t = fminf(fmaxf(t, 0.0f), tmax);
+    b = min((int)t, nb - 2);
+    f = t - (float)b;
+}
+
 // Where the rows of a local proposal come from: the shared-memory ring or, when the ring is off, the
 // packed table in L2.  slot0 = ring slot of column j = split of the step being evaluated.
 struct RowSource {
@@ -162,56 +183,125 @@ struct RowSource {
     int ring_cols, ring_rows, span, slot0;
 };
 
-// sum over the pairs (i, j), ilo <= i < split <= j <= jhi, j - i >= min_sep, of e(new) - e(old); the candidate
-// C-beta of residue j is (nx, ny, nz)[j - joff].  Work is dealt to `nthr` threads, this one being `tid`.
-template <bool RING>
-__device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSource &rs, const float *cbx, const float *cby,
-                                                 const float *cbz, const float *nx, const float *ny, const float *nz,
-                                                 int joff, int ilo, int split, int jhi, int tid, int nthr)
+// floor(a / b) for 0 <= a < 2^16, 1 <= b < 2^10 without the integer-division sequence
+__device__ __forceinline__ int small_div(int a, int b)
 {
-    const int nI = split - ilo, nJ = jhi - split + 1;
+    return __float2int_rd(__fdividef((float)a + 0.5f, (float)b));
+}
+
+// row index of the pair i < j in 32 bits (L < 46341)
+__device__ __forceinline__ int tri_row(int i, int j, int L) { return (i * (2 * L - i - 1)) / 2 - i - 1 + j; }
+
+// sum over the pairs (i, j), ilo <= i < split <= j <= jhi, j - i >= min_sep, of e(new) - e(old), where new = the
+// C-beta of j turned by R.  Work is dealt to `nthr` threads, this one being `tid`: a thread OWNS a column j -
+// it turns CB_j itself (fp64, rounded once to fp32) and keeps both positions in registers - and walks the rows
+// i; when a round has fewer columns than threads, S threads share a column and take every S-th row.
+template <bool RING>
+__device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSource &rs, const float4 *cb4,
+                                                 const double *Xcb, const double *Ycb, const double *Zcb, const Rot &R,
+                                                 int ilo, int split, int jhi, int tid, int nthr)
+{
+    const int nJ = jhi - split + 1;
     double acc = 0.0;
-    if (nI <= 0 || nJ <= 0) return acc;
-    const int total = nI * nJ;
-    const int stepI = nthr / nJ, stepJ = nthr - stepI * nJ;
-    int ii = tid / nJ, jj = tid - ii * nJ;
-    for (int q = tid; q < total; q += nthr) {
-        const int i = ilo + ii, j = split + jj;
-        if (j - i >= m.min_sep) {
-            const float xi = cbx[i], yi = cby[i], zi = cbz[i];
-            float dx = xi - nx[j - joff], dy = yi - ny[j - joff], dz = zi - nz[j - joff];
-            const float d2n = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-            dx = xi - cbx[j]; dy = yi - cby[j]; dz = zi - cbz[j];
-            const float d2o = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-            // a pair beyond the last bin centre before and after scores the same clamped value twice:
-            // its term is exactly 0 and its row is never touched
-            if (d2n < m.far2 || d2o < m.far2) {
-                float en, eo;
-                if (RING) {
-                    int slot = rs.slot0 + jj;                      // nJ <= w + 1 < ring_cols: one wrap at most
-                    if (slot >= rs.ring_cols) slot -= rs.ring_cols;
-                    const float *rowp = rs.ring + ((size_t)slot * rs.ring_rows + (i - j + rs.span)) * m.row_stride;
-                    en = pair_energy_row(rowp, d2n, m.c0, m.inv_delta, m.tmax, m.nb);
-                    eo = pair_energy_row(rowp, d2o, m.c0, m.inv_delta, m.tmax, m.nb);
-                } else {
-                    const float2 *rowp = m.Epk + (tri_base(i, m.L) + j) * m.nb;
-                    en = pair_energy(rowp, d2n, m.c0, m.inv_delta, m.tmax, m.nb);
-                    eo = pair_energy(rowp, d2o, m.c0, m.inv_delta, m.tmax, m.nb);
+    if (split <= ilo || nJ <= 0) return acc;
+    for (int c0 = 0; c0 < nJ; c0 += nthr) {
+        const int nc = min(nthr, nJ - c0);
+        int S = 1, col = tid, slice = 0;
+        if (nc < nthr) {
+            S = small_div(nthr, nc); slice = small_div(tid, nc); col = tid - slice * nc;
+            if (slice >= S) break;
+        }
+        const int j = split + c0 + col;
+        double x, y, z;
+        rot_apply(R, Xcb[j], Ycb[j], Zcb[j], x, y, z);
+        const float xn = (float)x, yn = (float)y, zn = (float)z;
+        const float4 o = cb4[j];
+        const int i_end = min(split - 1, j - m.min_sep);
+        const float *colp = nullptr;
+        if (RING) {
+            int slot = rs.slot0 + (j - split);               // nJ <= w + 1 < ring_cols: one wrap at most
+            if (slot >= rs.ring_cols) slot -= rs.ring_cols;
+            colp = rs.ring + ((size_t)slot * rs.ring_rows + (rs.span - j)) * m.row_stride;   // + i * row_stride
+        }
+        // U rows per trip: all distances first, then all gathers, then the sums, so that a thread has 2U loads in
+        // flight instead of stalling on each pair's row (the rows of near pairs come from L2, ~600 cycles away)
+        constexpr int U = 4;
+        for (int i = ilo + slice; i <= i_end; i += U * S) {
+            float d2n[U], d2o[U];
+            int iu[U];
+            bool near[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int ii = i + u * S;
+                const bool valid = ii <= i_end;
+                iu[u] = valid ? ii : i;
+                const float4 ci = cb4[iu[u]];
+                float dx = ci.x - xn, dy = ci.y - yn, dz = ci.z - zn;
+                d2n[u] = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                dx = ci.x - o.x; dy = ci.y - o.y; dz = ci.z - o.z;
+                d2o[u] = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                // a pair beyond the last bin centre before and after scores the same clamped value twice:
+                // its term is exactly 0 and its row is never touched
+                near[u] = valid && (d2n[u] < m.far2 || d2o[u] < m.far2);
+            }
+            float fn[U], fo[U];
+            int bn[U], bo[U];
+            if (RING) {
+                float en0[U], en1[U], eo0[U], eo1[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    en0[u] = en1[u] = eo0[u] = eo1[u] = 0.0f;
+                    if (near[u]) {
+                        lerp_coords(d2n[u], m.c0, m.inv_delta, m.tmax, m.nb, bn[u], fn[u]);
+                        lerp_coords(d2o[u], m.c0, m.inv_delta, m.tmax, m.nb, bo[u], fo[u]);
+                        const float *rowp = colp + iu[u] * m.row_stride;
+                        en0[u] = rowp[bn[u]]; en1[u] = rowp[bn[u] + 1];
+                        eo0[u] = rowp[bo[u]]; eo1[u] = rowp[bo[u] + 1];
+                    }
                 }
-                acc += (double)(en - eo);
+#pragma unroll
+                for (int u = 0; u < U; ++u)
+                    if (near[u]) acc += (double)(fmaf(fn[u], en1[u] - en0[u], en0[u]) - fmaf(fo[u], eo1[u] - eo0[u], eo0[u]));
+            } else {
+                float2 vn[U], vo[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    vn[u] = vo[u] = make_float2(0.0f, 0.0f);
+                    if (near[u]) {
+                        lerp_coords(d2n[u], m.c0, m.inv_delta, m.tmax, m.nb, bn[u], fn[u]);
+                        lerp_coords(d2o[u], m.c0, m.inv_delta, m.tmax, m.nb, bo[u], fo[u]);
+                        const float2 *rowp = m.Epk + (size_t)tri_row(iu[u], j, m.L) * m.nb;
+                        vn[u] = __ldg(rowp + bn[u]); vo[u] = __ldg(rowp + bo[u]);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u)
+                    if (near[u]) acc += (double)(fmaf(fn[u], vn[u].y, vn[u].x) - fmaf(fo[u], vo[u].y, vo[u].x));
             }
         }
-        ii += stepI; jj += stepJ;
-        if (jj >= nJ) { jj -= nJ; ++ii; }
     }
     return acc;
 }
 
 // V (Eq. 3a) of the team's chain from its fp32 C-betas; every thread of the team returns the same value
-__device__ __forceinline__ double team_full_energy(const DevModel &m, const float *cbx, const float *cby, const float *cbz,
-                                                   double *red, int warp, int nwarps, int lane, int bar_id)
+__device__ __forceinline__ double team_full_energy(const DevModel &m, const float4 *cb4, double *red, int warp, int nwarps,
+                                                   int lane, int bar_id)
 {
-    double e = warp_sum(energy_range_cta(m, cbx, cby, cbz, 0, m.L - 1, warp, nwarps, lane));
+    double e = 0.0;
+    for (int i = warp; i < m.L - m.min_sep; i += nwarps) {
+        const float4 ci = cb4[i];
+        const int rb = tri_row(i, 0, m.L);
+#pragma unroll 2
+        for (int j = i + m.min_sep + lane; j < m.L; j += 32) {
+            const float4 cj = cb4[j];
+            const float dx = ci.x - cj.x, dy = ci.y - cj.y, dz = ci.z - cj.z;
+            const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+            // far pairs take the clamped value from the compact array (coalesced in j), near pairs gather their row
+            e += (double)((d2 >= m.far2) ? __ldg(m.Elast + rb + j)
+                                         : pair_energy(m.Epk + (size_t)(rb + j) * m.nb, d2, m.c0, m.inv_delta, m.tmax, m.nb));
+        }
+    }
+    e = warp_sum(e);
     if (lane == 0) red[warp] = e;
     team_bar(bar_id, nwarps * 32);
     double tot = 0.0;
@@ -230,7 +320,6 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     const int warp = warp_cta - slot * W;                 // warp within the team
     const int tid = warp * 32 + lane, nthreads = W * 32, nwarps = W;
     const int bar_id = 1 + slot;
-    const int wcap = sweep_wcap(L, a.window);
     const int span = min(2 * a.window, L - 1);            // largest j - i of an in-window pair
     const bool use_ring = R > 0;
 
@@ -259,36 +348,31 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
         if (!use_ring) return;
         const uint32_t row_bytes = (uint32_t)(m.row_stride * sizeof(float));
         long long q0 = 0;                                   // running number of column j = 0 of the sweep
+        int s = 0;                                          // ring slot of the next column
         for (long long t = a.sweep_offset; t < a.sweep_offset + a.n_sweeps; ++t) {
             if (sweep_is_global(t)) continue;
             for (int j = 0; j < L; ++j) {
                 const long long q = q0 + j;
-                if (lane == 0) {                            // slot q mod R is free once every team has passed column q - R
+                if (lane == 0) {                            // slot s is free once every team has passed column q - R
                     for (;;) {
                         long long mn = 0x7fffffffffffffffLL;
                         for (int g = 0; g < nvalid; ++g) mn = min(mn, prog[g]);
                         if (q - R < mn) break;
                         __nanosleep(40);
                     }
-                }
-                __syncwarp();
-                const int i_lo = max(0, j - span), i_hi = j - m.min_sep;
-                const int nrows = i_hi - i_lo + 1;
-                const int s = (int)(q % R);
-                void *bar = &full_bar[s];
-                if (lane == 0) {
+                    const int i_lo = max(0, j - span), i_hi = j - m.min_sep;
+                    const int nrows = i_hi - i_lo + 1;
+                    void *bar = &full_bar[s];
                     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the teams' reads of the old column come first
                     if (nrows > 0) mbar_expect_tx(bar, (uint32_t)nrows * row_bytes);
                     else mbar_arrive(bar);
-                }
-                __syncwarp();
-                // one lane issues the copies of the column: the operands of a bulk copy live in uniform registers,
-                // so a lane-divergent issue loop would be serialised lane by lane anyway
-                if (lane == 0)
+                    // one lane issues the copies of the column: the operands of a bulk copy live in uniform registers
                     for (int i = i_lo; i <= i_hi; ++i)
                         tma_bulk_g2s(ring + ((size_t)s * a.ring_rows + (i - j + span)) * m.row_stride,
-                                     m.Epl + (size_t)(tri_base(i, L) + j) * m.row_stride, row_bytes, bar);
+                                     m.Epl + (size_t)tri_row(i, j, L) * m.row_stride, row_bytes, bar);
+                }
                 __syncwarp();
+                if (++s == R) s = 0;
             }
             q0 += L;
         }
@@ -297,16 +381,15 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     if (slot >= nvalid) return;
 
     // ================= team: one chain =====================================================================
-    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L, a.window, W);
+    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L);
     double *X = reinterpret_cast<double *>(cbase), *Y = X + 4 * L, *Z = Y + 4 * L;
     double *red = Z + 4 * L, *b_cd = red + kMaxWarps, *b_sd = b_cd + kDrawBatch, *b_lu = b_sd + kDrawBatch;
-    double *rot_s = b_lu + kDrawBatch, *sp_dE = rot_s + 12 * kMaxWarps;
-    float *cbx = reinterpret_cast<float *>(sp_dE + kMaxWarps), *cby = cbx + L, *cbz = cby + L;
-    float *nwx = cbz + L, *nwy = nwx + L, *nwz = nwy + L;
-    float *s = nwz + L;
+    double *rot_s = b_lu + kDrawBatch, *sp_dE = rot_s + 12 * kMaxSpec;
+    float4 *cb4 = reinterpret_cast<float4 *>(sp_dE + kMaxSpec);
+    float *s = reinterpret_cast<float *>(cb4 + L);
     float *b_sp = s + n;
-    float *lnw = b_sp + kDrawBatch;
-    int *sp_acc = reinterpret_cast<int *>(lnw + (size_t)nwarps * 3 * wcap);
+    int *sp_acc = reinterpret_cast<int *>(b_sp + kDrawBatch);
+    const double *Xcb = X + 3 * L, *Ycb = Y + 3 * L, *Zcb = Z + 3 * L;
 
     const long long row = row0 + slot;
     const unsigned long long chain = (unsigned long long)(a.chain_offset + row);
@@ -315,33 +398,48 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     team_bar(bar_id, nthreads);
     if (warp == 0)
         nerf_build_warp(m, s, lane, [&](int res, int at, double x, double y, double z) {
-            const int f = 4 * res + at;
+            const int f = at * L + res;
             X[f] = x; Y[f] = y; Z[f] = z;
-            if (at == 3) { cbx[res] = (float)x; cby[res] = (float)y; cbz[res] = (float)z; }
+            if (at == 3) cb4[res] = make_float4((float)x, (float)y, (float)z, 0.0f);
         });
     team_bar(bar_id, nthreads);
 
     double best = INFINITY, e_end = 0.0;
     unsigned long long acc_l = 0, acc_g = 0;
-    const int nspec = max(1, min(nwarps, a.spec_local > 0 ? a.spec_local : nwarps));
+    // local proposals are evaluated by groups of gl lanes, 32 / gl groups per warp
+    const int gshift = a.lanes_per_step == 8 ? 3 : (a.lanes_per_step == 16 ? 4 : 5);
+    const int gl = 1 << gshift, gpw = 32 >> gshift;
+    const int grp = lane >> gshift, glane = lane & (gl - 1);
+    int nspec = max(1, min(min(nwarps * gpw, kMaxSpec), a.spec_local > 0 ? a.spec_local : kMaxSpec));
+    // a pass may not reach beyond what the ring can hold next to the window (else the team would wait for a column
+    // whose slot it still occupies itself)
+    if (use_ring) nspec = max(1, min(nspec, 2 * (R - min(a.window, L - 1) - 2) - 1));
     const int draw_warp_u = nwarps > 1 ? 1 : 0;              // the warp that draws the uniforms of the accept test
     long long q0 = 0;                                        // running column number of j = 0 (local sweeps)
+    int seen_slot = R - 1;                                   // ring slot and phase parity of the last column waited for
+    uint32_t seen_par = 1;
     RowSource rs;
     rs.ring = use_ring ? ring : nullptr; rs.ring_cols = R; rs.ring_rows = a.ring_rows; rs.span = span; rs.slot0 = 0;
 
     // the bond the torsion k turns about: phi_c N->CA, psi_c CA->C
     auto step_rot = [&](int k, int bi) -> Rot {
-        const int fa = 4 * (k >> 1) + (k & 1), fb = fa + 1;
+        const int fa = (k & 1) * L + (k >> 1), fb = fa + L;
         return rot_about(X[fa], Y[fa], Z[fa], X[fb], Y[fb], Z[fb], b_cd[bi], b_sd[bi], (k & 1) ? m.inv_len_ca_c : m.inv_len_n_ca);
     };
-    // the accepted rotation moves every atom bonded after the turned bond
+    // the accepted rotation moves every atom bonded after the turned bond: phi_c moves C_c, CB_c and all later
+    // residues; psi_c moves the residues after c (R19)
     auto commit = [&](const Rot &R_, int k) {
-        const int m0 = 4 * (k >> 1) + 2 + 2 * (k & 1);       // first flat atom that moves
-        for (int f = m0 + tid; f < 4 * L; f += nthreads) {
-            double x, y, z;
-            rot_apply(R_, X[f], Y[f], Z[f], x, y, z);
-            X[f] = x; Y[f] = y; Z[f] = z;
-            if ((f & 3) == 3) { cbx[f >> 2] = (float)x; cby[f >> 2] = (float)y; cbz[f >> 2] = (float)z; }
+        const int c = k >> 1;
+#pragma unroll
+        for (int at = 0; at < 4; ++at) {
+            const int r0 = ((k & 1) == 0 && at >= 2) ? c : c + 1;
+            for (int res = r0 + tid; res < L; res += nthreads) {
+                const int f = at * L + res;
+                double x, y, z;
+                rot_apply(R_, X[f], Y[f], Z[f], x, y, z);
+                X[f] = x; Y[f] = y; Z[f] = z;
+                if (at == 3) cb4[res] = make_float4((float)x, (float)y, (float)z, 0.0f);
+            }
         }
     };
 
@@ -353,33 +451,38 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
         else if (t >= a.ramp_sweeps - 1) T = a.t_end;
         else T = a.t_start * pow(a.t_end / a.t_start, (double)t / (double)(a.ramp_sweeps - 1));
         const double invT = 1.0 / T;
-        long long seen = q0 - 1;                             // last ring column this team has waited for
+        int seen_rel = -1;                                   // last column of this sweep the team has waited for
+        const int slot_j0 = (seen_slot + 1 == R) ? 0 : seen_slot + 1;   // ring slot of column 0 of this sweep
 
         int k = 0, batch_start = 0, batch_end = 0;
         while (k < n) {
-            // ---- a1/a2: draws of the next 32 steps, one lane per step (R5-R7) -----------------------------
+            // ---- a1/a2: draws of the next 64 steps, two per lane (R5-R7) ----------------------------------
             if (k >= batch_end) {
                 batch_start = k; batch_end = min(n, k + kDrawBatch);
-                const int kk = k + lane;
-                if (kk < n && (warp == 0 || warp == draw_warp_u)) {
-                    const unsigned long long step = (unsigned long long)t * (unsigned long long)n + (unsigned long long)kk;
-                    if (warp == 0) {
-                        const uint32_t x0 = draw0(a.seed, chain, step, PURPOSE_PROPOSAL);
-                        float sp;
-                        if (a.prop_mode == 1) {
-                            const int mm = (int)(x0 % (uint32_t)a.grid);
-                            sp = __fmul_rn(__fdiv_rn((float)(2 * mm - a.grid), (float)a.grid), 3.14159274101257324f);
-                        } else {
-                            const int h = (int)(x0 >> 8) - (1 << 23);
-                            sp = __fmul_rn((float)h * 1.1920928955078125e-07f, 3.14159274101257324f);
+                if (warp == 0 || warp == draw_warp_u) {
+#pragma unroll 1
+                    for (int bi = lane; bi < kDrawBatch; bi += 32) {
+                        const int kk = k + bi;
+                        if (kk >= n) break;
+                        const unsigned long long step = (unsigned long long)t * (unsigned long long)n + (unsigned long long)kk;
+                        if (warp == 0) {
+                            const uint32_t x0 = draw0(a.seed, chain, step, PURPOSE_PROPOSAL);
+                            float sp;
+                            if (a.prop_mode == 1) {
+                                const int mm = (int)(x0 % (uint32_t)a.grid);
+                                sp = __fmul_rn(__fdiv_rn((float)(2 * mm - a.grid), (float)a.grid), 3.14159274101257324f);
+                            } else {
+                                const int h = (int)(x0 >> 8) - (1 << 23);
+                                sp = __fmul_rn((float)h * 1.1920928955078125e-07f, 3.14159274101257324f);
+                            }
+                            double sd, cd;
+                            sincos((double)sp - (double)s[kk], &sd, &cd);
+                            b_sp[bi] = sp; b_cd[bi] = cd; b_sd[bi] = sd;
                         }
-                        double sd, cd;
-                        sincos((double)sp - (double)s[kk], &sd, &cd);
-                        b_sp[lane] = sp; b_cd[lane] = cd; b_sd[lane] = sd;
-                    }
-                    if (warp == draw_warp_u) {
-                        const uint32_t x0 = draw0(a.seed, chain, step, PURPOSE_ACCEPT);
-                        b_lu[lane] = log((double)((x0 >> 8) + 1u) * 5.9604644775390625e-08);
+                        if (warp == draw_warp_u) {
+                            const uint32_t x0 = draw0(a.seed, chain, step, PURPOSE_ACCEPT);
+                            b_lu[bi] = log((double)((x0 >> 8) + 1u) * 5.9604644775390625e-08);
+                        }
                     }
                 }
                 team_bar(bar_id, nthreads);
@@ -387,21 +490,22 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
             if (is_global) {
                 // ======== one proposal, evaluated by the whole team ========================================
                 const int bi = k - batch_start;
-                const int c = k >> 1, split = c + (k & 1);
+                const int split = (k >> 1) + (k & 1);
                 const bool inert = (k == 0) || (k == n - 1);
                 double dE = 0.0;
-                Rot Rk;
                 if (!inert) {
-                    // ---- a3: rotation of the right-hand side about the flipped bond ------------------------
-                    Rk = step_rot(k, bi);
-                    for (int j = split + tid; j < L; j += nthreads) {
-                        double x, y, z;
-                        rot_apply(Rk, X[4 * j + 3], Y[4 * j + 3], Z[4 * j + 3], x, y, z);
-                        nwx[j] = (float)x; nwy[j] = (float)y; nwz[j] = (float)z;
+                    // ---- a3/a5/a6: turn the right-hand side about the flipped bond, cross pairs, reduction ------
+                    double acc;
+                    {
+                        const Rot Rk = step_rot(k, bi);
+                        if (tid == 0) {                       // kept in shared memory for the commit, not in registers
+#pragma unroll
+                            for (int q = 0; q < 9; ++q) rot_s[q] = Rk.r[q];
+#pragma unroll
+                            for (int q = 0; q < 3; ++q) rot_s[9 + q] = Rk.t[q];
+                        }
+                        acc = warp_sum(cross_pairs_dE<false>(m, rs, cb4, Xcb, Ycb, Zcb, Rk, 0, split, L - 1, tid, nthreads));
                     }
-                    team_bar(bar_id, nthreads);
-                    // ---- a5/a6: cross pairs, then the reduction -------------------------------------------
-                    double acc = warp_sum(cross_pairs_dE<false>(m, rs, cbx, cby, cbz, nwx, nwy, nwz, 0, 0, split, L - 1, tid, nthreads));
                     if (lane == 0) red[warp] = acc;
                     team_bar(bar_id, nthreads);
                     for (int w = 0; w < nwarps; ++w) dE += red[w];
@@ -420,57 +524,64 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 if (accept) {
                     ++acc_g;
                     if (tid == 0) s[k] = b_sp[bi];
-                    if (!inert) commit(Rk, k);
+                    if (!inert) {
+                        Rot Rc;
+#pragma unroll
+                        for (int q = 0; q < 9; ++q) Rc.r[q] = rot_s[q];
+#pragma unroll
+                        for (int q = 0; q < 3; ++q) Rc.t[q] = rot_s[9 + q];
+                        commit(Rc, k);
+                    }
                 }
                 team_bar(bar_id, nthreads);
                 ++k;
             } else {
-                // ======== up to nspec proposals, warp r evaluating step k + r against the current state ====
+                // ======== up to nspec proposals, group r evaluating step k + r against the current state ===
                 const int S = min(nspec, batch_end - k);
                 if (use_ring) {
                     // columns left of the window centre are dead for this chain; wait for the ones the pass needs
                     if (tid == 0) prog[slot] = q0 + (k >> 1);
-                    const long long need = q0 + min(L - 1, ((k + S - 1) >> 1) + a.window);
-                    while (seen < need) {
-                        ++seen;
-                        mbar_wait(&full_bar[seen % R], (uint32_t)((seen / R) & 1));
+                    const int need = min(L - 1, ((k + S - 1) >> 1) + a.window);
+                    while (seen_rel < need) {
+                        ++seen_rel;
+                        if (++seen_slot == R) { seen_slot = 0; seen_par ^= 1u; }
+                        mbar_wait(&full_bar[seen_slot], seen_par);
                     }
                 }
-                if (warp < S) {
-                    const int kk = k + warp, bi = kk - batch_start;
+                const int r = warp * gpw + grp;
+                const bool active = r < S;
+                const int kk = k + r, bi = kk - batch_start;
+                const bool inert = (kk == 0) || (kk == n - 1);
+                double dE = 0.0;
+                Rot Rk;
+                if (active && !inert) {
                     const int c = kk >> 1, split = c + (kk & 1);
-                    const bool inert = (kk == 0) || (kk == n - 1);
-                    double dE = 0.0;
-                    Rot Rk;
-                    if (!inert) {
-                        Rk = step_rot(kk, bi);
-                        const int ilo = max(0, c - a.window), jhi = min(L - 1, c + a.window);
-                        float *px = lnw + (size_t)warp * 3 * wcap, *py = px + wcap, *pz = py + wcap;
-                        for (int j = split + lane; j <= jhi; j += 32) {
-                            double x, y, z;
-                            rot_apply(Rk, X[4 * j + 3], Y[4 * j + 3], Z[4 * j + 3], x, y, z);
-                            px[j - split] = (float)x; py[j - split] = (float)y; pz[j - split] = (float)z;
-                        }
-                        __syncwarp();
-                        // ---- a4/a6: in-window cross pairs (Eq. 3b), warp reduction ------------------------
-                        if (use_ring) rs.slot0 = (int)((q0 + split) % R);
-                        dE = warp_sum(use_ring ? cross_pairs_dE<true>(m, rs, cbx, cby, cbz, px, py, pz, split, ilo, split, jhi, lane, 32)
-                                               : cross_pairs_dE<false>(m, rs, cbx, cby, cbz, px, py, pz, split, ilo, split, jhi, lane, 32));
+                    Rk = step_rot(kk, bi);
+                    const int ilo = max(0, c - a.window), jhi = min(L - 1, c + a.window);
+                    // ---- a4: in-window cross pairs (Eq. 3b) -------------------------------------------------
+                    if (use_ring) {
+                        rs.slot0 = slot_j0 + split;
+                        if (rs.slot0 >= R) rs.slot0 %= R;
+                        dE = cross_pairs_dE<true>(m, rs, cb4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane, gl);
+                    } else {
+                        dE = cross_pairs_dE<false>(m, rs, cb4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane, gl);
                     }
-                    if (lane == 0) {
-                        sp_dE[warp] = dE;
-                        sp_acc[warp] = (b_lu[bi] <= -dE * invT) ? 1 : 0;   // Eq. 2a, R14
-                        if (!inert) {
+                }
+                // ---- a6: reduction over the group's lanes (every lane of the warp takes part) ----------------
+                for (int d = gl >> 1; d > 0; d >>= 1) dE += __shfl_xor_sync(0xffffffffu, dE, d);
+                if (active && glane == 0) {
+                    sp_dE[r] = dE;
+                    sp_acc[r] = (b_lu[bi] <= -dE * invT) ? 1 : 0;   // Eq. 2a, R14
+                    if (!inert) {
 #pragma unroll
-                            for (int q = 0; q < 9; ++q) rot_s[12 * warp + q] = Rk.r[q];
+                        for (int q = 0; q < 9; ++q) rot_s[12 * r + q] = Rk.r[q];
 #pragma unroll
-                            for (int q = 0; q < 3; ++q) rot_s[12 * warp + 9 + q] = Rk.t[q];
-                        }
+                        for (int q = 0; q < 3; ++q) rot_s[12 * r + 9 + q] = Rk.t[q];
                     }
                 }
                 team_bar(bar_id, nthreads);
-                int rsel = S;                                 // first accepted step of the pass
-                for (int q = S - 1; q >= 0; --q) if (sp_acc[q]) rsel = q;
+                int rsel = 0;                                 // first accepted step of the pass
+                while (rsel < S && !sp_acc[rsel]) ++rsel;
                 const int nstand = (rsel < S) ? rsel + 1 : S; // steps whose result stands
                 if (tid < nstand) {
                     const long long q = (t - a.sweep_offset) * n + k + tid;
@@ -487,12 +598,12 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                     ++acc_l;
                     if (tid == 0) s[kc] = b_sp[kc - batch_start];
                     if (kc != 0 && kc != n - 1) {
-                        Rot Rk;
+                        Rot Rc;
 #pragma unroll
-                        for (int q = 0; q < 9; ++q) Rk.r[q] = rot_s[12 * rsel + q];
+                        for (int q = 0; q < 9; ++q) Rc.r[q] = rot_s[12 * rsel + q];
 #pragma unroll
-                        for (int q = 0; q < 3; ++q) Rk.t[q] = rot_s[12 * rsel + 9 + q];
-                        commit(Rk, kc);
+                        for (int q = 0; q < 3; ++q) Rc.t[q] = rot_s[12 * rsel + 9 + q];
+                        commit(Rc, kc);
                     }
                 }
                 team_bar(bar_id, nthreads);
@@ -504,7 +615,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
             if (use_ring && tid == 0) prog[slot] = q0;       // every column of this sweep is dead for this chain
         }
         // ---- a9: book-keeping at the sweep end ----------------------------------------------------
-        e_end = team_full_energy(m, cbx, cby, cbz, red, warp, nwarps, lane, bar_id);
+        e_end = team_full_energy(m, cb4, red, warp, nwarps, lane, bar_id);
         if (e_end < best) {
             best = e_end;
             if (a.best_state)
@@ -512,7 +623,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
         }
         if (tid == 0 && a.first_hit && (float)e_end <= a.energy_threshold) atomicMin(a.first_hit, (unsigned long long)t);
     }
-    if (a.n_sweeps == 0) e_end = team_full_energy(m, cbx, cby, cbz, red, warp, nwarps, lane, bar_id);
+    if (a.n_sweeps == 0) e_end = team_full_energy(m, cb4, red, warp, nwarps, lane, bar_id);
     for (int q = tid; q < n; q += nthreads) a.states[row * n + q] = s[q];
     if (tid == 0) {
         if (a.energy) a.energy[row] = (float)e_end;
