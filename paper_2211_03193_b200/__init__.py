@@ -72,10 +72,11 @@ def lib():
     """Load csrc/libamh_b200.so (fails loudly when it has not been built)."""
     global _lib
     if _lib is None:
-        if not os.path.exists(_build.LIB):
+        path = os.environ.get("AMH_B200_LIB", _build.LIB)      # another build of the same library (kernel experiments)
+        if not os.path.exists(path):
             raise ImportError("%s is missing: run `python -m paper_2211_03193_b200.build` (nvcc, sm_100a); "
-                              "there is no CPU fallback" % _build.LIB)
-        L = C.CDLL(_build.LIB)
+                              "there is no CPU fallback" % path)
+        L = C.CDLL(path)
         L.amh_last_error.restype = C.c_char_p
         L.amh_version.restype = C.c_char_p
         L.amh_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int,

@@ -404,7 +404,7 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
                     c->m.L, sc->window, sh.C, sh.W, sh.smem, c->max_smem);
     a.C = sh.C; a.W = sh.W; a.ring_cols = sh.R; a.ring_rows = sh.ring_rows;
     a.spec_local = c->opt.spec_local;
-    a.lanes_per_step = c->opt.lanes_per_step > 0 ? c->opt.lanes_per_step : 16;
+    a.lanes_per_step = c->opt.lanes_per_step > 0 ? c->opt.lanes_per_step : 8;
     const long long ctas = (B + sh.C - 1) / sh.C;
     amh::sweep_kernel<<<(unsigned)ctas, 32 * (sh.C * sh.W + 1), sh.smem, st>>>(c->m, a);
     AMH_CUDA(cudaGetLastError());
