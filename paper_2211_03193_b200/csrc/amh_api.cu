@@ -305,20 +305,19 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
         return w_eff + 3 + amh::kMaxSpec / 2 + (C > 1 ? 4 : 0);    // + reach of a speculative pass + drift between teams
     };
     auto fits = [&](int C, int, int R) { return amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride) <= budget; };
-    // chains per CTA: spread the batch over the SMs, one CTA each
+    // chains per CTA: spread the batch over the SMs (one CTA each) and keep as many teams resident as shared memory
+    // allows; the ring is added only when it fits beside them (warps in flight are worth more than the ring)
     int C = c->opt.chains_per_cta;
-    if (C <= 0) C = (int)std::min<long long>(8, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));
+    if (C <= 0) {
+        C = (int)std::min<long long>(8, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));
+        while (C > 1 && !fits(C, 0, 0)) --C;
+    }
     int W = c->opt.warps_per_chain;
-    auto auto_w = [&](int C_) { return std::max(1, std::min(amh::kMaxTeamWarps / C_, 8)); };
-    int R;
-    for (;;) {
-        const int Wc = W > 0 ? std::max(1, std::min(W, amh::kMaxTeamWarps / C)) : auto_w(C);
-        R = ring_for(C);
-        if (fits(C, Wc, R)) { W = Wc; break; }
-        if (c->opt.chains_per_cta <= 0 && C > 1) { --C; continue; }
-        R = 0;                                               // the ring does not fit: rows are gathered from L2
-        W = Wc;
-        break;
+    W = W > 0 ? std::max(1, std::min(W, amh::kMaxTeamWarps / C)) : std::max(1, std::min(amh::kMaxTeamWarps / C, 8));
+    int R = ring_for(C);
+    if (R > 0 && !fits(C, W, R)) {
+        R = ring_for(1);                                     // without the slack for drift between teams
+        if (!fits(C, W, R)) R = 0;                           // the ring does not fit: rows are gathered from L2
     }
     sh.C = C; sh.W = W; sh.R = R;
     if (R == 0) sh.ring_rows = 0;

@@ -288,17 +288,38 @@ __device__ __forceinline__ double team_full_energy(const DevModel &m, const floa
                                                    int lane, int bar_id)
 {
     double e = 0.0;
+    constexpr int U = 4;                                     // columns per trip: all gathers of a trip in flight together
     for (int i = warp; i < m.L - m.min_sep; i += nwarps) {
         const float4 ci = cb4[i];
         const int rb = tri_row(i, 0, m.L);
-#pragma unroll 2
-        for (int j = i + m.min_sep + lane; j < m.L; j += 32) {
-            const float4 cj = cb4[j];
-            const float dx = ci.x - cj.x, dy = ci.y - cj.y, dz = ci.z - cj.z;
-            const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+        for (int j0 = i + m.min_sep + lane; j0 < m.L; j0 += 32 * U) {
+            float d2[U], v[U], f[U];
+            float2 g[U];
+            bool far[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int j = min(j0 + 32 * u, m.L - 1);
+                const float4 cj = cb4[j];
+                const float dx = ci.x - cj.x, dy = ci.y - cj.y, dz = ci.z - cj.z;
+                d2[u] = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                far[u] = d2[u] >= m.far2;
+            }
             // far pairs take the clamped value from the compact array (coalesced in j), near pairs gather their row
-            e += (double)((d2 >= m.far2) ? __ldg(m.Elast + rb + j)
-                                         : pair_energy(m.Epk + (size_t)(rb + j) * m.nb, d2, m.c0, m.inv_delta, m.tmax, m.nb));
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int j = j0 + 32 * u;
+                v[u] = 0.0f; g[u] = make_float2(0.0f, 0.0f); f[u] = 0.0f;
+                if (j < m.L) {
+                    if (far[u]) v[u] = __ldg(m.Elast + rb + j);
+                    else {
+                        int b;
+                        lerp_coords(d2[u], m.c0, m.inv_delta, m.tmax, m.nb, b, f[u]);
+                        g[u] = __ldg(m.Epk + (size_t)(rb + j) * m.nb + b);
+                    }
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) e += (double)(far[u] ? v[u] : fmaf(f[u], g[u].y, g[u].x));
         }
     }
     e = warp_sum(e);
