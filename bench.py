@@ -78,6 +78,18 @@ def run_kwargs(cfg: gi.Config, B: int, chain_offset: int):
     return kw
 
 
+def shard(cfg: gi.Config, rank: int, world: int):
+    """Chain sharding: rank r runs chains [r B, (r+1) B) of a world*B batch - weak scaling,
+    no data-path collective.  Returns (chain_offset, start states, run kwargs) of this rank."""
+    off = rank * cfg.B
+    return off, gi.initial_states(cfg.B, cfg.n, seed=1, chain_offset=off), run_kwargs(cfg, cfg.B, off)
+
+
+def job_rate(world: int, proposals_per_rank: int, steps: int, max_total_ms: float) -> float:
+    """Whole-job proposals/s: the units all ranks processed / the slowest rank's device time."""
+    return world * proposals_per_rank * steps / (max_total_ms * 1e-3)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
@@ -166,6 +178,25 @@ def oracle_leg(cfg: gi.Config, sample_chains: int, sample_sweeps: int, steps: in
                        % (sample_chains, sample_sweeps, cfg.name, props)), t
 
 
+def oracle_threshold(cfg: gi.Config, runs: int = 10, proposals: int = 100000):
+    """Energy threshold of the time-to-threshold metric (protocol of PAPER.md:184-188): the oracle
+    runs `runs` single chains of `proposals` proposals each under the config's schedule, one core per chain; E* = mean
+    of their minimum sweep-end energies, cpu_s = wall time of those runs."""
+    import oracle
+    oracle.build()
+    ref = gi.reference_torsions(cfg.L, cfg.cfg_seed)
+    CB = oracle.coords(ref)[3]
+    D = np.linalg.norm(CB[:, None] - CB[None], axis=-1)
+    m = oracle.Model(gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi), gi.bin_edges(cfg.n_bins, cfg.d_lo, cfg.d_hi))
+    sweeps = max(1, -(-proposals // cfg.n))
+    s0 = gi.initial_states(runs, cfg.n, seed=1)
+    t0 = time.perf_counter()
+    r = m.run(s0, sweeps, **run_kwargs(cfg, runs, 0))
+    dt = time.perf_counter() - t0
+    return dict(threshold=float(np.mean(r["best_energy"])), cpu_s=dt, cpu_runs=runs, cpu_sweeps_per_run=sweeps,
+                cpu_cores=min(runs, oracle.num_threads()))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -241,16 +272,20 @@ def main():
                                                spec_local=args.spec_local, ring_cols=args.ring_cols,
                                                lanes_per_step=args.lanes_per_step))
     del p
-    chain_offset = rank * B
-    s0_host = torch.from_numpy(gi.initial_states(B, n, seed=1, chain_offset=chain_offset)).pin_memory()
+    chain_offset, s0_np, kw = shard(cfg, rank, world)
+    s0_host = torch.from_numpy(s0_np).pin_memory()
     s0_dev = s0_host.cuda()
     states = torch.empty_like(s0_dev)
-    kw = run_kwargs(cfg, B, chain_offset)
     if "per_chain_T" in kw:
         kw["per_chain_T"] = torch.from_numpy(kw["per_chain_T"]).cuda()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
     stream = torch.cuda.current_stream()
     info = g.launch_info(B, cfg.window)
+
+    tts = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        tts = oracle_threshold(cfg)
+        kw["energy_threshold"] = tts["threshold"]
 
     def one_step():
         states.copy_(s0_dev)
@@ -279,8 +314,16 @@ def main():
     total_ms = float(tmax.item())
     ms_per_step = total_ms / args.steps
     props_per_step = world * cfg.proposals
-    value = props_per_step / (ms_per_step * 1e-3)
+    value = job_rate(world, cfg.proposals, args.steps, total_ms)
     best = float(res["best_energy"].min().item()) if res is not None else None
+    if tts is not None:
+        hit = int(res["first_hit_sweep"].item())
+        tts.update(first_hit_sweep=hit, gpu_s=(ms_per_step * 1e-3 * (hit + 1) / cfg.n_sweeps) if hit >= 0 else None,
+                   protocol="E* = mean over 10 oracle chains (100,000 proposals each, this config's schedule) of the minimum "
+                            "sweep-end energy; gpu_s = step time x (first sweep at whose end some chain of the batch has V <= E*, "
+                            "+ 1) / sweeps; cpu_s = wall time of the oracle runs, one core per chain")
+        tts["speedup_vs_oracle"] = (tts["cpu_s"] / tts["gpu_s"]) if tts["gpu_s"] else None
+        kw.pop("energy_threshold")
 
     # ---------------- e2e: the same step through amh_run_host, pinned host buffers ----------------
     e2e = None
@@ -334,7 +377,7 @@ def main():
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
                 data="synthetic", config=workload, clocks=clocks, e2e=e2e, gpu_launches=launches,
-                roofline=roofline, cpu_baseline=cpu_baseline)
+                roofline=roofline, cpu_baseline=cpu_baseline, time_to_threshold=tts)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -139,6 +139,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
         const double c_last = e0 + ((double)n_bins - 0.5) * delta;
         const double lim = c_last * (1.0 + 1e-5) + 1e-5 * delta;
         m.far2 = std::nextafter((float)(lim * lim), INFINITY);
+        m.dfar = std::nextafter((float)std::sqrt((double)m.far2), INFINITY);
     }
     m.A = mplus(o.ang_n_ca_c, 0.0, o.len_ca_c);
     m.W = mplus(o.ang_c_n_ca, o.omega, o.len_n_ca);

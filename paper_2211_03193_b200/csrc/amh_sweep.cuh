@@ -53,6 +53,7 @@ struct RunArgs {
 constexpr int kDrawBatch = 64;           // steps whose draws are generated together, two per lane
 constexpr int kMaxWarps = 16;            // array bound of the per-warp scratch of a team
 constexpr int kMaxSpec = 16;             // local proposals evaluated per pass, at most
+constexpr int kBlk = 8;                  // residues per culling block of the global phase
 constexpr int kMaxTeamWarps = 15;        // team warps per CTA: chains x warps per chain (+ the producer = 512 threads)
 constexpr int kMaxChains = 15;           // chains per CTA (named barriers 1..15)
 constexpr int kSweepMaxThreads = 512;    // 15 team warps + the producer: 128 registers per thread
@@ -61,11 +62,12 @@ constexpr int kSweepMaxThreads = 512;    // 15 team warps + the producer: 128 re
 //   double X[4L], Y[4L], Z[4L]   atoms, index atom * L + res (atom 0..3 = N, CA, C, CB)
 //   double red[16], b_cd[64], b_sd[64], b_lu[64], rot_s[16][12], sp_dE[16]
 //   float4 cb4[L]                fp32 copy of the C-betas (what the pair loops read)
+//   float4 blk4[ceil(L/8)]       bounding spheres of 8-residue blocks (culling in the global phase)
 //   float  s[n], b_sp[64];  int sp_acc[16]
 __host__ __device__ inline size_t chain_smem_bytes(int L)
 {
     const size_t doubles = 12 * (size_t)L + kMaxWarps + 3 * kDrawBatch + 12 * kMaxSpec + kMaxSpec;
-    size_t floats = 4 * (size_t)L + 2 * (size_t)L + kDrawBatch + kMaxSpec;
+    size_t floats = 4 * (size_t)L + 4 * (((size_t)L + kBlk - 1) / kBlk) + 2 * (size_t)L + kDrawBatch + kMaxSpec;
     floats = (floats + 3) & ~(size_t)3;
     return sizeof(double) * doubles + sizeof(float) * floats;
 }
@@ -196,8 +198,8 @@ __device__ __forceinline__ int tri_row(int i, int j, int L) { return (i * (2 * L
 // C-beta of j turned by R.  Work is dealt to `nthr` threads, this one being `tid`: a thread OWNS a column j -
 // it turns CB_j itself (fp64, rounded once to fp32) and keeps both positions in registers - and walks the rows
 // i; when a round has fewer columns than threads, S threads share a column and take every S-th row.
-template <bool RING>
-__device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSource &rs, const float4 *cb4,
+template <bool RING, bool CULL>
+__device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSource &rs, const float4 *cb4, const float4 *blk4,
                                                  const double *Xcb, const double *Ycb, const double *Zcb, const Rot &R,
                                                  int ilo, int split, int jhi, int tid, int nthr)
 {
@@ -226,13 +228,13 @@ __device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSou
         // U rows per trip: all distances first, then all gathers, then the sums, so that a thread has 2U loads in
         // flight instead of stalling on each pair's row (the rows of near pairs come from L2, ~600 cycles away)
         constexpr int U = 4;
-        for (int i = ilo + slice; i <= i_end; i += U * S) {
+        auto trip = [&](int i, int stride) {
             float d2n[U], d2o[U];
             int iu[U];
             bool near[U];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int ii = i + u * S;
+                const int ii = i + u * stride;
                 const bool valid = ii <= i_end;
                 iu[u] = valid ? ii : i;
                 const float4 ci = cb4[iu[u]];
@@ -278,9 +280,49 @@ __device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSou
                 for (int u = 0; u < U; ++u)
                     if (near[u]) acc += (double)(fmaf(fn[u], vn[u].y, vn[u].x) - fmaf(fo[u], vo[u].y, vo[u].x));
             }
+        };
+        if (CULL) {
+            // rows in blocks of kBlk consecutive residues (ilo = 0): a block whose bounding sphere lies beyond the last
+            // bin centre of BOTH positions of CB_j holds only pairs whose term is exactly 0, and is skipped whole;
+            // the S threads that share a column take every S-th block
+            const int nblk = i_end < 0 ? 0 : i_end / kBlk + 1;
+            for (int b = slice; b < nblk; b += S) {
+                const float4 bl = blk4[b];
+                float dx = bl.x - xn, dy = bl.y - yn, dz = bl.z - zn;
+                const float dn = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                dx = bl.x - o.x; dy = bl.y - o.y; dz = bl.z - o.z;
+                const float dq = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                if (dn >= bl.w && dq >= bl.w) continue;
+#pragma unroll
+                for (int t = 0; t < kBlk / U; ++t)
+                    if (b * kBlk + t * U <= i_end) trip(b * kBlk + t * U, 1);
+            }
+        } else {
+            for (int i = ilo + slice; i <= i_end; i += U * S) trip(i, S);
         }
     }
     return acc;
+}
+
+// bounding spheres of the blocks [first, last] of kBlk consecutive C-betas: blk4[b] = {centre, ((dfar + radius)(1 + 1e-5))^2}
+__device__ __forceinline__ void team_blocks(const DevModel &m, const float4 *cb4, float4 *blk4, int first, int tid, int nthr)
+{
+    const int nblk = (m.L + kBlk - 1) / kBlk;
+    for (int b = first + tid; b < nblk; b += nthr) {
+        const int lo = b * kBlk, hi = min(m.L, lo + kBlk);
+        float cx = 0.0f, cy = 0.0f, cz = 0.0f;
+        for (int i = lo; i < hi; ++i) { const float4 c = cb4[i]; cx += c.x; cy += c.y; cz += c.z; }
+        const float inv = 1.0f / (float)(hi - lo);
+        cx *= inv; cy *= inv; cz *= inv;
+        float r2 = 0.0f;
+        for (int i = lo; i < hi; ++i) {
+            const float4 c = cb4[i];
+            const float dx = c.x - cx, dy = c.y - cy, dz = c.z - cz;
+            r2 = fmaxf(r2, fmaf(dx, dx, fmaf(dy, dy, dz * dz)));
+        }
+        const float t = (m.dfar + sqrtf(r2)) * 1.00001f + 1e-4f;
+        blk4[b] = make_float4(cx, cy, cz, t * t);
+    }
 }
 
 // V (Eq. 3a) of the team's chain from its fp32 C-betas; every thread of the team returns the same value
@@ -407,7 +449,8 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     double *red = Z + 4 * L, *b_cd = red + kMaxWarps, *b_sd = b_cd + kDrawBatch, *b_lu = b_sd + kDrawBatch;
     double *rot_s = b_lu + kDrawBatch, *sp_dE = rot_s + 12 * kMaxSpec;
     float4 *cb4 = reinterpret_cast<float4 *>(sp_dE + kMaxSpec);
-    float *s = reinterpret_cast<float *>(cb4 + L);
+    float4 *blk4 = cb4 + L;
+    float *s = reinterpret_cast<float *>(blk4 + (L + kBlk - 1) / kBlk);
     float *b_sp = s + n;
     int *sp_acc = reinterpret_cast<int *>(b_sp + kDrawBatch);
     const double *Xcb = X + 3 * L, *Ycb = Y + 3 * L, *Zcb = Z + 3 * L;
@@ -475,6 +518,10 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
         int seen_rel = -1;                                   // last column of this sweep the team has waited for
         const int slot_j0 = (seen_slot + 1 == R) ? 0 : seen_slot + 1;   // ring slot of column 0 of this sweep
 
+        if (is_global) {                                     // the local sweeps moved everything: fresh culling blocks
+            team_blocks(m, cb4, blk4, 0, tid, nthreads);
+            team_bar(bar_id, nthreads);
+        }
         int k = 0, batch_start = 0, batch_end = 0;
         while (k < n) {
             // ---- a1/a2: draws of the next 64 steps, two per lane (R5-R7) ----------------------------------
@@ -525,7 +572,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
 #pragma unroll
                             for (int q = 0; q < 3; ++q) rot_s[9 + q] = Rk.t[q];
                         }
-                        acc = warp_sum(cross_pairs_dE<false>(m, rs, cb4, Xcb, Ycb, Zcb, Rk, 0, split, L - 1, tid, nthreads));
+                        acc = warp_sum(cross_pairs_dE<false, true>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, 0, split, L - 1, tid, nthreads));
                     }
                     if (lane == 0) red[warp] = acc;
                     team_bar(bar_id, nthreads);
@@ -552,6 +599,8 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
 #pragma unroll
                         for (int q = 0; q < 3; ++q) Rc.t[q] = rot_s[9 + q];
                         commit(Rc, k);
+                        team_bar(bar_id, nthreads);
+                        team_blocks(m, cb4, blk4, (k >> 1) / kBlk, tid, nthreads);
                     }
                 }
                 team_bar(bar_id, nthreads);
@@ -583,9 +632,9 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                     if (use_ring) {
                         rs.slot0 = slot_j0 + split;
                         if (rs.slot0 >= R) rs.slot0 %= R;
-                        dE = cross_pairs_dE<true>(m, rs, cb4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane, gl);
+                        dE = cross_pairs_dE<true, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane, gl);
                     } else {
-                        dE = cross_pairs_dE<false>(m, rs, cb4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane, gl);
+                        dE = cross_pairs_dE<false, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane, gl);
                     }
                 }
                 // ---- a6: reduction over the group's lanes (every lane of the warp takes part) ----------------
