@@ -5,15 +5,18 @@
 // Chains are independent: teams never wait for one another except through the ring.
 //
 // Global sweeps (Eq. 1, 3a): the team evaluates one proposal at a time over its O(L^2/6) straddling
-// pairs; rows of far pairs are never touched, near pairs gather 8 bytes from the packed table in L2.
+// pairs.  A thread owns a column j: it turns CB_j itself and walks the rows i in blocks of 8; a block
+// whose bounding sphere is beyond the last bin centre for both positions of CB_j is skipped whole, pairs
+// clamped before and after are skipped one by one (their term is exactly 0), near pairs gather 8 bytes
+// from the packed table in L2, four rows' gathers in flight at a time.
 //
 // Local sweeps (Eq. 2, 3b): a proposal has only ~65-150 pairs, and Alg. 1 orders the proposals of a
 // chain strictly.
 //   * Speculation.  The draws are counter-based (R6), so the proposals of steps k, k+1, ... are known in
-//     advance: warp r of the team evaluates step k+r AGAINST THE CURRENT STATE, and the results are
-//     consumed in order up to and including the first accepted step; later results were computed against
-//     a state that no longer exists and are thrown away (their steps are evaluated again in the next
-//     pass).  The trajectory is exactly the sequential one.
+//     advance: GROUP r (8, 16 or 32 lanes; up to 16 groups per team) evaluates step k+r AGAINST THE
+//     CURRENT STATE, and the results are consumed in order up to and including the first accepted step;
+//     later results were computed against a state that no longer exists and are thrown away (their steps
+//     are evaluated again in the next pass).  The trajectory is exactly the sequential one.
 //   * Table ring.  Every chain of the CTA walks k = 0..n-1, so they all need the same table rows at about
 //     the same time: pair (i, j) is needed while the window centre c is in [max(i, j-w), min(j, i+w)].
 //     The producer streams "column" j = the rows (i, j), j-2w <= i <= j-min_sep, into slot q mod R of a
