@@ -41,7 +41,7 @@ typedef struct amh_ctx amh_ctx;   /* opaque; owns the device energy table and th
 typedef enum {
     AMH_OK = 0,
     AMH_ERR_INVALID_ARG = 1,   /* NULL where a pointer is required, sizes < 1, T <= 0, NaN/Inf/negative p, ... */
-    AMH_ERR_UNSUPPORTED = 2,   /* non-uniform bins, AMH_PARAM_TR5, L beyond the shared-memory plan, Gaussian proposals */
+    AMH_ERR_UNSUPPORTED = 2,   /* non-uniform bins, AMH_PARAM_TR5, L beyond the shared-memory plan */
     AMH_ERR_CUDA = 3,          /* a CUDA runtime call failed; see amh_last_error() */
     AMH_ERR_OOM = 4
 } amh_status;
@@ -91,11 +91,16 @@ typedef struct {
 
 typedef enum {
     AMH_PROP_UNIFORM = 0,   /* s'_k = fp32(h * 2^-23) * fp32(pi), h = (x0 >> 8) - 2^23    (BASELINE.json configs; R5) */
-    AMH_PROP_GRID = 1       /* s'_k = fp32((2m - G)/G) * fp32(pi), m = x0 mod G           (tests: Boltzmann pins P4/P5) */
-    /* the paper's Gaussian single flip is DESIGN.md NEXT-1: AMH_ERR_UNSUPPORTED */
+    AMH_PROP_GRID = 1,      /* s'_k = fp32((2m - G)/G) * fp32(pi), m = x0 mod G           (tests: Boltzmann pins P4/P5) */
+    AMH_PROP_GAUSSIAN = 2   /* the paper's single flip (Eq. 1b, 129, 145): s'_k = wrap(s_k + sigma_t z),
+                               z = sqrt(-2 ln u1) cos(2 pi u2) (Box-Muller), u1 = ((x0 >> 8) + 1) 2^-24, u2 = (x1 >> 8) 2^-24,
+                               evaluated in fp64, wrapped to [-pi, pi), rounded once to fp32 */
 } amh_prop_mode;
 
-typedef struct { int mode; int grid; } amh_proposal;
+/* sigma_t = sigma_start + (sigma_end - sigma_start) * t / (ramp_sweeps - 1) for absolute sweep index t (the paper
+ * anneals 10 -> 4 degrees over a run), clamped to sigma_end for t >= ramp_sweeps - 1; sigma_start ==
+ * sigma_end or ramp_sweeps <= 1 means constant.  Radians, > 0; read in Gaussian mode only. */
+typedef struct { int mode; int grid; double sigma_start, sigma_end; long long ramp_sweeps; } amh_proposal;
 
 /* Results of amh_run.  Every pointer is optional (NULL = not wanted).  DEVICE memory for amh_run,
  * HOST memory for amh_run_host.  B = rows of the batch, n = 2L. */

@@ -194,8 +194,10 @@ class Model:
     def follow(self, states, steps, forced_acc, *, n_global=1, n_local=10, window=8, global_first=True,
                t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
                sigma_start=0.0, sigma_end=0.0, ramp_sigma=0, seed=1, chain_offset=0, sweep_offset=0,
-               n_threads=0):
-        """Follow mode: replay `steps` proposals taking the decisions in forced_acc [B][steps]."""
+               n_threads=0, forced_prop=None):
+        """Follow mode: replay `steps` proposals taking the decisions in forced_acc [B][steps]; with
+        forced_prop [B][steps] also the proposed values (Gaussian mode, R5) - "prop" in the result
+        is still this implementation's own proposal."""
         s = np.array(states, dtype=np.float32, order="C").reshape(-1, self.n)
         B = s.shape[0]
         fa = np.ascontiguousarray(forced_acc, dtype=np.uint8).reshape(B, steps)
@@ -207,8 +209,9 @@ class Model:
         dE = np.zeros((B, steps))
         g = np.zeros((B, steps))
         acc = np.zeros((B, steps), np.uint8)
+        fp = None if forced_prop is None else np.ascontiguousarray(forced_prop, dtype=np.float32).reshape(B, steps)
         rc = lib().amho_follow(C.byref(self._m), C.byref(prm), _p(s), C.c_longlong(B), C.c_int(steps),
-                               _p(fa), _p(prop), _p(dE), _p(g), _p(acc))
+                               _p(fa), _p(fp), _p(prop), _p(dE), _p(g), _p(acc))
         if rc != 0:
             raise ValueError("amho_follow: invalid argument")
         return dict(states=s, prop=prop, dE=dE, g=g, acc=acc)

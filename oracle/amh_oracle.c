@@ -394,10 +394,15 @@ int amho_run(const amho_model *m, const amho_run_params *p, float *states, long 
 /* Follow mode: replay the first `steps` proposals of
  * a run with sweep_offset as given, taking at every step the decision in `forced_acc` (the other
  * implementation's accept bits) while recording this implementation's own proposal, dE, gap g and
- * decision from the SHARED current state.  states is [B][n], in/out (ends at the forced path). */
+ * decision from the SHARED current state.  states is [B][n], in/out (ends at the forced path).
+ * forced_prop (may be NULL): the other implementation's proposed values.  DESIGN.md R5: a Gaussian
+ * proposal goes through log/sqrt/cos, which two math libraries round differently in the last place,
+ * so there the replay is teacher-forced - this implementation still records its OWN proposal in
+ * own_prop (the test checks it within 2 ulp) but evaluates and applies the forced value, so that
+ * both stay on one path.  For UNIFORM and GRID the two are bit-identical and NULL is passed. */
 int amho_follow(const amho_model *m, const amho_run_params *p, float *states, long long B, int steps,
-                const unsigned char *forced_acc, float *own_prop, double *own_dE, double *own_g,
-                unsigned char *own_acc)
+                const unsigned char *forced_acc, const float *forced_prop, float *own_prop, double *own_dE,
+                double *own_g, unsigned char *own_acc)
 {
     const int L = m->L, n = 2 * L;
     if (L < 1 || p->n_global + p->n_local <= 0) return 1;
@@ -418,11 +423,12 @@ int amho_follow(const amho_model *m, const amho_run_params *p, float *states, lo
                 const int k = (int)(step % (uint64_t)n);
                 const int is_global = phase_is_global(p, t);
                 const double T = amho_temperature(p, t, row);
-                const float s_new = propose(p, chain, step, t, s[k]);
+                size_t z = (size_t)row * steps + q;
+                const float s_own = propose(p, chain, step, t, s[k]);
+                const float s_new = forced_prop ? forced_prop[z] : s_own;
                 const double dE = proposal_dE(m, p, is_global, k, s, s_new, CB, CBn);
                 const double lu = log(uniform01(p, chain, step));
-                size_t z = (size_t)row * steps + q;
-                own_prop[z] = s_new; own_dE[z] = dE; own_g[z] = lu + dE / T;
+                own_prop[z] = s_own; own_dE[z] = dE; own_g[z] = lu + dE / T;
                 own_acc[z] = (unsigned char)(lu <= -dE / T);
                 if (forced_acc[z]) s[k] = s_new;
             }

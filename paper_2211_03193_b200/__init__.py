@@ -18,9 +18,9 @@ import numpy as np
 from . import build as _build
 
 __all__ = ["AMH", "AMHError", "Options", "lib", "lib_path", "default_options", "philox4x32_10",
-           "PROP_UNIFORM", "PROP_GRID", "EXPORTS"]
+           "PROP_UNIFORM", "PROP_GRID", "PROP_GAUSSIAN", "EXPORTS"]
 
-PROP_UNIFORM, PROP_GRID = 0, 1
+PROP_UNIFORM, PROP_GRID, PROP_GAUSSIAN = 0, 1, 2
 
 # every symbol include/amh.h declares
 EXPORTS = ["amh_default_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
@@ -51,7 +51,8 @@ class _Temperature(C.Structure):
 
 
 class _Proposal(C.Structure):
-    _fields_ = [("mode", C.c_int), ("grid", C.c_int)]
+    _fields_ = [("mode", C.c_int), ("grid", C.c_int), ("sigma_start", C.c_double), ("sigma_end", C.c_double),
+                ("ramp_sweeps", C.c_longlong)]
 
 
 class _Outputs(C.Structure):
@@ -221,13 +222,14 @@ class AMH:
     # ---- amh_run ---------------------------------------------------------------------------------
     @staticmethod
     def _structs(n_global, n_local, window, global_first, t_start, t_end, ramp_sweeps, per_chain_T_ptr,
-                 prop_mode, grid):
+                 prop_mode, grid, sigma_start=0.0, sigma_end=0.0, ramp_sigma=0):
         return (_Schedule(n_global, n_local, window, int(bool(global_first))),
                 _Temperature(t_start, t_end, ramp_sweeps, per_chain_T_ptr),
-                _Proposal(prop_mode, grid))
+                _Proposal(prop_mode, grid, sigma_start, sigma_end, ramp_sigma))
 
     def run(self, states, n_sweeps: int, *, n_global=1, n_local=10, window=8, global_first=True,
             t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
+            sigma_start=0.0, sigma_end=0.0, ramp_sigma=0,
             seed=1, chain_offset=0, sweep_offset=0, trace_steps=0, energy_threshold=None,
             want=("energy", "best_energy", "best_state", "n_accept_local", "n_accept_global"), stream=None):
         """amh_run on a DEVICE batch; `states` (torch.float32 [B][n], cuda) is updated in place.
@@ -264,7 +266,8 @@ class AMH:
             if pct.numel() != B:
                 raise ValueError("per_chain_T must have B entries")
         sc, tp, pr = self._structs(n_global, n_local, window, global_first, t_start, t_end, ramp_sweeps,
-                                   pct.data_ptr() if pct is not None else None, prop_mode, grid)
+                                   pct.data_ptr() if pct is not None else None, prop_mode, grid,
+                                   sigma_start, sigma_end, ramp_sigma)
         _check(lib().amh_run(self._h, s.data_ptr(), B, int(n_sweeps), int(sweep_offset), int(chain_offset),
                              C.byref(sc), C.byref(tp), C.byref(pr), int(seed), C.byref(o), _stream_ptr(stream)))
         r["_keepalive"] = pct
@@ -272,6 +275,7 @@ class AMH:
 
     def run_host(self, states: np.ndarray, n_sweeps: int, *, n_global=1, n_local=10, window=8, global_first=True,
                  t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
+                 sigma_start=0.0, sigma_end=0.0, ramp_sigma=0,
                  seed=1, chain_offset=0, sweep_offset=0, trace_steps=0, energy_threshold=None,
                  want=("energy", "best_energy")):
         """amh_run_host: HOST numpy buffers in and out (states updated in place); synchronous."""
@@ -302,7 +306,8 @@ class AMH:
         if per_chain_T is not None:
             pct = np.ascontiguousarray(per_chain_T, dtype=np.float32)
         sc, tp, pr = self._structs(n_global, n_local, window, global_first, t_start, t_end, ramp_sweeps,
-                                   pct.ctypes.data if pct is not None else None, prop_mode, grid)
+                                   pct.ctypes.data if pct is not None else None, prop_mode, grid,
+                                   sigma_start, sigma_end, ramp_sigma)
         _check(lib().amh_run_host(self._h, s.ctypes.data, B, int(n_sweeps), int(sweep_offset), int(chain_offset),
                                   C.byref(sc), C.byref(tp), C.byref(pr), int(seed), C.byref(o), _stream_ptr()))
         return r

@@ -367,9 +367,11 @@ static amh_status check_run(const amh_ctx *c, const float *states, long long B, 
     if (!tp->per_chain_T && !(tp->t_start > 0.0 && tp->t_end > 0.0 && std::isfinite(tp->t_start) && std::isfinite(tp->t_end)))
         return fail(AMH_ERR_INVALID_ARG, "amh_run: temperatures must be finite and > 0");
     if (pr) {
-        if (pr->mode == 2) return fail(AMH_ERR_UNSUPPORTED, "amh_run: Gaussian proposals are not built (DESIGN.md NEXT-1)");
-        if (pr->mode != AMH_PROP_UNIFORM && pr->mode != AMH_PROP_GRID) return fail(AMH_ERR_INVALID_ARG, "amh_run: unknown proposal mode %d", pr->mode);
+        if (pr->mode != AMH_PROP_UNIFORM && pr->mode != AMH_PROP_GRID && pr->mode != AMH_PROP_GAUSSIAN)
+            return fail(AMH_ERR_INVALID_ARG, "amh_run: unknown proposal mode %d", pr->mode);
         if (pr->mode == AMH_PROP_GRID && (pr->grid < 1 || pr->grid > (1 << 20))) return fail(AMH_ERR_INVALID_ARG, "amh_run: grid = %d out of range", pr->grid);
+        if (pr->mode == AMH_PROP_GAUSSIAN && !(pr->sigma_start > 0.0 && pr->sigma_end > 0.0 && std::isfinite(pr->sigma_start) && std::isfinite(pr->sigma_end)))
+            return fail(AMH_ERR_INVALID_ARG, "amh_run: Gaussian proposals need finite sigma_start, sigma_end > 0");
     }
     if (out && out->trace_steps < 0) return fail(AMH_ERR_INVALID_ARG, "amh_run: trace_steps < 0");
     return AMH_OK;
@@ -388,6 +390,7 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     a.n_global = sc->n_global; a.n_local = sc->n_local; a.window = sc->window; a.global_first = sc->global_first ? 1 : 0;
     a.t_start = tp->t_start; a.t_end = tp->t_end; a.ramp_sweeps = tp->ramp_sweeps; a.per_chain_T = tp->per_chain_T;
     a.prop_mode = pr ? pr->mode : AMH_PROP_UNIFORM; a.grid = pr ? pr->grid : 0;
+    a.sigma_start = pr ? pr->sigma_start : 0.0; a.sigma_end = pr ? pr->sigma_end : 0.0; a.ramp_sigma = pr ? pr->ramp_sweeps : 0;
     a.seed = seed;
     if (out) {
         a.energy = out->energy; a.best_energy = out->best_energy; a.best_state = out->best_state;

@@ -74,6 +74,17 @@ __device__ __forceinline__ uint32_t draw0(unsigned long long seed, unsigned long
     return x[0];
 }
 
+// words 0 (returned) and 1 of the same block
+__device__ __forceinline__ uint32_t draw01(unsigned long long seed, unsigned long long chain,
+                                           unsigned long long step, uint32_t purpose, uint32_t &x1)
+{
+    uint32_t x[4];
+    philox4x32_10((uint32_t)step, (uint32_t)(step >> 32), (uint32_t)chain, purpose,
+                  (uint32_t)seed, (uint32_t)(seed >> 32), x);
+    x1 = x[1];
+    return x[0];
+}
+
 // ------------------------------------------------------------------------------------------------
 // Rigid transforms (fp64)
 // ------------------------------------------------------------------------------------------------

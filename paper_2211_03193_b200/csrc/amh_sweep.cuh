@@ -36,6 +36,8 @@ struct RunArgs {
     long long ramp_sweeps;
     const float *per_chain_T;
     int prop_mode, grid;
+    double sigma_start, sigma_end;       // Gaussian mode: linear ramp over ramp_sigma sweeps
+    long long ramp_sigma;
     // launch shape
     int C, W;                            // chains per CTA, warps per chain
     int spec_local;                      // local proposals evaluated per pass (<= W * 32 / lanes_per_step, <= 16)
@@ -105,8 +107,9 @@ __device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
     const uint32_t a = smem_u32(bar);
     uint32_t ok;
     do {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        // the last operand lets the hardware park the thread for up to ~1 us instead of spinning on the barrier
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity), "r"(1000u) : "memory");
     } while (!ok);
 }
 // global -> shared bulk copy (TMA, no tensor map); bytes is a multiple of 16, both addresses 16-byte aligned
@@ -424,7 +427,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                         long long mn = 0x7fffffffffffffffLL;
                         for (int g = 0; g < nvalid; ++g) mn = min(mn, prog[g]);
                         if (q - R < mn) break;
-                        __nanosleep(40);
+                        __nanosleep(200);
                     }
                     const int i_lo = max(0, j - span), i_hi = j - m.min_sep;
                     const int nrows = i_hi - i_lo + 1;
@@ -518,6 +521,10 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
         else if (t >= a.ramp_sweeps - 1) T = a.t_end;
         else T = a.t_start * pow(a.t_end / a.t_start, (double)t / (double)(a.ramp_sweeps - 1));
         const double invT = 1.0 / T;
+        double sigma_t = a.sigma_start;                      // Gaussian mode: linear in the sweep index
+        if (!(a.sigma_start == a.sigma_end || a.ramp_sigma <= 1 || t <= 0))
+            sigma_t = (t >= a.ramp_sigma - 1) ? a.sigma_end
+                                              : a.sigma_start + (a.sigma_end - a.sigma_start) * ((double)t / (double)(a.ramp_sigma - 1));
         int seen_rel = -1;                                   // last column of this sweep the team has waited for
         const int slot_j0 = (seen_slot + 1 == R) ? 0 : seen_slot + 1;   // ring slot of column 0 of this sweep
 
@@ -537,9 +544,19 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                         if (kk >= n) break;
                         const unsigned long long step = (unsigned long long)t * (unsigned long long)n + (unsigned long long)kk;
                         if (warp == 0) {
-                            const uint32_t x0 = draw0(a.seed, chain, step, PURPOSE_PROPOSAL);
+                            uint32_t x1;
+                            const uint32_t x0 = draw01(a.seed, chain, step, PURPOSE_PROPOSAL, x1);
                             float sp;
-                            if (a.prop_mode == 1) {
+                            if (a.prop_mode == 2) {
+                                // the paper's Gaussian flip: Box-Muller in fp64, wrapped to [-pi, pi)
+                                const double u1 = ((double)(x0 >> 8) + 1.0) * 5.9604644775390625e-08;
+                                const double u2 = (double)(x1 >> 8) * 5.9604644775390625e-08;
+                                const double z = sqrt(-2.0 * log(u1)) * cos(6.283185307179586 * u2);
+                                double v = (double)s[kk] + sigma_t * z;
+                                v -= 6.283185307179586 * floor((v + 3.141592653589793) / 6.283185307179586);
+                                sp = (float)v;
+                                if (sp >= 3.14159274101257324f) sp -= 2.0f * 3.14159274101257324f;
+                            } else if (a.prop_mode == 1) {
                                 const int mm = (int)(x0 % (uint32_t)a.grid);
                                 sp = __fmul_rn(__fdiv_rn((float)(2 * mm - a.grid), (float)a.grid), 3.14159274101257324f);
                             } else {

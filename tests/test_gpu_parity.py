@@ -232,6 +232,37 @@ def test_trajectory_parity_ramp_per_chain_T_and_offset(amh, orc, torch, synth, g
     assert acc[7] > acc[0]                    # the hot replica accepts more
 
 
+def test_trajectory_parity_gaussian_proposals(amh, orc, torch, synth, gpu_model):
+    # NEXT-1: the paper's Gaussian single flip with sigma annealed 10 -> 4 degrees.
+    # log/sqrt/cos differ in the last place between CUDA's and the host's math library, so the replay is
+    # teacher-forced (R5): the oracle's own proposal must be within 2 fp32 ulp of the kernel's (or the same
+    # angle on the other side of the +-pi cut), then both continue from the kernel's value.
+    L, B, sweeps = 48, 16, 8
+    ref, p, edges, m = synth(L, 1000)
+    g = gpu_model(L, 1000)
+    s0 = gi.initial_states(B, 2 * L, seed=21)
+    steps = sweeps * 2 * L
+    kw = dict(n_global=1, n_local=3, window=5, seed=31, prop_mode=amh.PROP_GAUSSIAN, sigma_start=math.radians(10),
+              sigma_end=math.radians(4), ramp_sigma=sweeps, chain_offset=2)
+    st = torch.from_numpy(s0.copy()).cuda()
+    r = g.run(st, sweeps, trace_steps=steps, **kw)
+    acc = r["trace_acc"].cpu().numpy(); prop = r["trace_prop"].cpu().numpy(); dE = r["trace_dE"].cpu().numpy()
+    f = m.follow(s0, steps, acc, forced_prop=prop, **kw)
+    d = np.abs(prop.astype(np.float64) - f["prop"].astype(np.float64))
+    d = np.minimum(d, np.abs(d - 2 * math.pi))
+    assert d.max() <= 2 * np.spacing(np.float32(math.pi)), d.max()
+    assert np.all((prop >= -np.float32(math.pi)) & (prop < np.float32(math.pi)))
+    diff = acc != f["acc"]
+    assert np.all(np.abs(f["g"][diff]) < 1e-4)
+    assert np.abs(dE - f["dE"]).max() < 2e-3
+    assert np.array_equal(st.cpu().numpy(), f["states"])
+    # small steps are accepted far more often than uniform resampling: the accept/commit path is exercised
+    assert acc.mean() > 0.3
+    e = r["energy"].cpu().numpy().astype(np.float64)
+    want = m.energy(st.cpu().numpy())
+    assert np.all(np.abs(e - want) < 1e-5 * np.abs(want))
+
+
 @pytest.mark.parametrize("L", [2, 3, 5])
 def test_tiny_chains_run(amh, orc, torch, synth, gpu_model, L):
     # degenerate sizes: L < min_sep + 1 has no pairs (every proposal accepted); window clamps at both ends

@@ -248,3 +248,45 @@ def test_follow_mode_reproduces_the_free_run(orc, synth):
     f2 = m.follow(s0, steps, forced, **kw)
     assert np.array_equal(f2["dE"][:, :31], r["trace_dE"][:, :31])
     assert not np.array_equal(f2["states"], f["states"])
+
+
+def test_gaussian_proposal_law_wrap_and_sigma_ramp(orc, synth):
+    # P8 (NEXT-1; Eq. 1b, 129, 145): s'_k = wrap(s_k + sigma_t z), z ~ N(0, 1) by Box-Muller.
+    # With every decision forced to "reject" the state never moves, so the recorded proposals expose z:
+    # its law is tested against the normal distribution (Kolmogorov-Smirnov), its symmetry is what Eq. 1a
+    # needs, the wrap keeps values in [-pi, pi) and is congruent mod 2 pi, and sigma_t hits both ends of its ramp.
+    L, B, sweeps = 16, 8, 64
+    n = 2 * L
+    steps = sweeps * n
+    ref, p, edges, m = synth(L, 1000)
+    none = np.zeros((B, steps), np.uint8)
+    s0 = np.full((B, n), 0.25, np.float32)
+    kw = dict(n_global=0, n_local=1, window=2, seed=9, prop_mode=orc.PROP_GAUSSIAN)
+    f = m.follow(s0, steps, none, sigma_start=0.3, sigma_end=0.3, **kw)
+    z = (f["prop"].astype(np.float64) - 0.25) / 0.3
+    assert np.array_equal(f["states"], s0)
+    assert stats.kstest(z.ravel(), "norm").pvalue > 0.01
+    assert abs(z.mean()) < 4.0 / math.sqrt(z.size) and abs(z.var() - 1.0) < 0.03
+    assert abs((z > 0).mean() - 0.5) < 4 * 0.5 / math.sqrt(z.size)                # symmetric proposal (Eq. 1b)
+    assert abs(np.corrcoef(z[:, :-1].ravel(), z[:, 1:].ravel())[0, 1]) < 0.02     # steps draw independently
+    assert not np.array_equal(z[0], z[1])                                        # chains draw independently
+    # wrap: the same draws from a start next to +pi land in [-pi, pi) and are congruent mod 2 pi
+    s1 = np.full((B, n), 3.1, np.float32)
+    f1 = m.follow(s1, steps, none, sigma_start=0.3, sigma_end=0.3, **kw)
+    v = f1["prop"].astype(np.float64)
+    assert np.all((v >= -math.pi - 1e-6) & (v < math.pi)) and (v < 0).mean() > 0.3
+    d = v - (np.float64(np.float32(3.1)) + 0.3 * z)
+    assert np.all(np.abs(d - 2 * math.pi * np.rint(d / (2 * math.pi))) < 1e-6)
+    # sigma ramp, linear in the sweep index (the paper anneals 10 -> 4 degrees over a run)
+    f2 = m.follow(s0, steps, none, sigma_start=math.radians(10), sigma_end=math.radians(4), ramp_sigma=sweeps, **kw)
+    dz = (f2["prop"].astype(np.float64) - 0.25).reshape(B, sweeps, n)
+    assert np.allclose(dz[:, 0] / math.radians(10), z.reshape(B, sweeps, n)[:, 0], atol=2e-6)
+    assert np.allclose(dz[:, -1] / math.radians(4), z.reshape(B, sweeps, n)[:, -1], atol=2e-6)
+    mid = sweeps // 2
+    sig_mid = math.radians(10) + (math.radians(4) - math.radians(10)) * mid / (sweeps - 1)
+    assert np.allclose(dz[:, mid] / sig_mid, z.reshape(B, sweeps, n)[:, mid], atol=2e-6)
+    # teacher forcing: a forced proposal replaces the own one in the state, the own one is still reported
+    forced = (f["prop"] + np.float32(0.01)).astype(np.float32)
+    allacc = np.ones((B, n), np.uint8)
+    f3 = m.follow(s0, n, allacc, sigma_start=0.3, sigma_end=0.3, forced_prop=forced[:, :n], **kw)
+    assert np.array_equal(f3["states"], forced[:, :n]) and np.array_equal(f3["prop"], f["prop"][:, :n])
