@@ -250,7 +250,9 @@ __device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSou
                 d2o[u] = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
                 // a pair beyond the last bin centre before and after scores the same clamped value twice:
                 // its term is exactly 0 and its row is never touched
-                near[u] = valid && (d2n[u] < m.far2 || d2o[u] < m.far2);
+                // (in the window of a local proposal nearly every pair is near: the test is skipped there and a far
+                // pair goes through the clamped interpolation, which gives the same two values and the same 0)
+                near[u] = valid && (!CULL || d2n[u] < m.far2 || d2o[u] < m.far2);
             }
             float fn[U], fo[U];
             int bn[U], bo[U];
