@@ -154,28 +154,36 @@ def profiled_traffic(cfg_name: str):
 
 
 # ------------------------------------------------------------------------------------------------
-def oracle_leg(cfg: gi.Config, sample_chains: int, sample_sweeps: int, steps: int = 1, warmup: int = 0):
-    """The fp64 oracle, as it stands, on the host cores, on a bounded sample of the workload."""
+def oracle_leg(cfg: gi.Config, steps: int = 1, warmup: int = 0, target_s: float = 15.0):
+    """The fp64 oracle, as it stands, on the host cores, on a bounded sample of the workload: the first 64 chains
+    of the batch for as many whole cycles of the schedule as fit in about `target_s` seconds of wall time per step
+    (sized from a two-cycle calibration run; at least two cycles, at most the config's sweep count)."""
     import oracle
     oracle.build()
     ref = gi.reference_torsions(cfg.L, cfg.cfg_seed)
     CB = oracle.coords(ref)[3]
     D = np.linalg.norm(CB[:, None] - CB[None], axis=-1)
     m = oracle.Model(gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi), gi.bin_edges(cfg.n_bins, cfg.d_lo, cfg.d_hi))
-    s0 = gi.initial_states(sample_chains, cfg.n, seed=1)
-    kw = run_kwargs(cfg, sample_chains, 0)
+    chains = min(cfg.B, 64)
+    s0 = gi.initial_states(chains, cfg.n, seed=1)
+    kw = run_kwargs(cfg, chains, 0)
+    cyc = cfg.n_global + cfg.n_local
+    t0 = time.perf_counter()
+    m.run(s0, min(cfg.n_sweeps, 2 * cyc), **kw)
+    t_cal = (time.perf_counter() - t0) / 2.0
+    sweeps = int(min(cfg.n_sweeps, cyc * max(2, int(target_s / max(t_cal, 1e-6)))))
     times = []
     for it in range(warmup + steps):
         t0 = time.perf_counter()
-        m.run(s0, sample_sweeps, **kw)
+        m.run(s0, sweeps, **kw)
         dt = time.perf_counter() - t0
         if it >= warmup:
             times.append(dt)
-    props = sample_chains * sample_sweeps * cfg.n
+    props = chains * sweeps * cfg.n
     t = float(np.mean(times))
     return dict(value=props / t, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
-                sample="%d chains x %d sweeps of %s (%d proposals per step, fp64, full rebuild + full re-sum per proposal)"
-                       % (sample_chains, sample_sweeps, cfg.name, props)), t
+                sample="%d chains x %d sweeps of %s (%d proposals, %.1f s per step, fp64, full rebuild + full re-sum per proposal)"
+                       % (chains, sweeps, cfg.name, props, t)), t
 
 
 def oracle_threshold(cfg: gi.Config, runs: int = 10, proposals: int = 100000):
@@ -233,8 +241,7 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return
-        sc, ss = min(cfg.B, 64), min(cfg.n_sweeps, 2 * (cfg.n_global + cfg.n_local))
-        cb, t = oracle_leg(cfg, sc, ss, steps=max(1, args.steps), warmup=args.warmup if args.warmup < 2 else 1)
+        cb, t = oracle_leg(cfg, steps=max(1, args.steps), warmup=min(args.warmup, 1))
         line = dict(impl="reference", metric=METRIC, value=cb["value"], unit=UNIT, n_gpus=0, steps=args.steps,
                     warmup=args.warmup, ms_per_step=t * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None,
                     dtype="f64", data="synthetic", config=workload, cpu_baseline=cb,
@@ -368,7 +375,7 @@ def main():
                     hbm_gbs_measured=peaks.get("hbm_gbs"))
     cpu_baseline = None
     if not args.no_cpu_baseline:
-        cpu_baseline, _ = oracle_leg(cfg, min(cfg.B, 64), min(cfg.n_sweeps, 2 * (cfg.n_global + cfg.n_local)))
+        cpu_baseline, _ = oracle_leg(cfg)
 
     workload.update(l2="flushed between timed steps (256 MiB write)", threads_per_chain=info["threads_per_chain"],
                     chains_per_cta=info["chains_per_cta"], ring_cols=info["ring_cols"], ring_rows=info["ring_rows"],
