@@ -153,25 +153,11 @@ __device__ __forceinline__ Rot rot_about(double ax, double ay, double az, double
     return R;
 }
 
-// the pair term from a plain row E[0..nb-1] in shared memory: the same fp32 operations, in the same order,
-// as pair_energy() on the packed row (E[b+1] - E[b] is formed here instead of at create)
-__device__ __forceinline__ float pair_energy_row(const float *row, float d2, float c0, float inv_delta, float tmax, int nb)
-{
-    const float d = sqrtf(d2);
-    float t = (d - c0) * inv_delta;
-    t = fminf(fmaxf(t, 0.0f), tmax);
-    int b = (int)t;
-    b = min(b, nb - 2);
-    const float f = t - (float)b;
-    const float e0 = row[b], e1 = row[b + 1];
-    return fmaf(f, e1 - e0, e0);
-}
-
-
 // bin index and fraction of R8's interpolation at squared distance d2.  d = sqrt(d2) by one reciprocal-square-root
 // and one Newton step: within 1 ulp of the correctly rounded root (the coordinates feeding d2
 // are themselves rounded to fp32), at 5 instructions instead of sqrtf()'s 9 with its special-case branch.  d2 = 0
-// (coincident atoms) is mapped to the first bin by the floor below.
+// (coincident atoms) is mapped to the first bin by the floor below.  Rows in the ring are plain E[0..nb-1]: the caller
+// forms E[b+1] - E[b] itself, the same fp32 subtraction the packed table did at create.
 __device__ __forceinline__ void lerp_coords(float d2, float c0, float inv_delta, float tmax, int nb, int &b, float &f)
 {
     d2 = fmaxf(d2, 1e-30f);
