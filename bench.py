@@ -329,8 +329,35 @@ def main():
                    protocol="E* = mean over 10 oracle chains (100,000 proposals each, this config's schedule) of the minimum "
                             "sweep-end energy; gpu_s = step time x (first sweep at whose end some chain of the batch has V <= E*, "
                             "+ 1) / sweeps; cpu_s = wall time of the oracle runs, one core per chain")
+        # nine more seeds (PAPER.md:184-188 takes means over repeated runs; median over 10 seeds),
+        # each run only long enough to see its hit
+        hits = [hit]
+        if hit >= 0:
+            short = int(min(cfg.n_sweeps, 8 * (hit + 1) + 4 * (cfg.n_global + cfg.n_local)))
+            for seed in range(2, 11):
+                states.copy_(torch.from_numpy(gi.initial_states(B, n, seed=seed, chain_offset=chain_offset)).cuda())
+                rr = g.run(states, short, want=("energy",), **dict(kw, seed=seed))
+                hits.append(int(rr["first_hit_sweep"].item()))
+            ok = sorted(h for h in hits if h >= 0)
+            med = ok[len(ok) // 2] if len(ok) == len(hits) else None
+            tts.update(first_hit_sweeps_10_seeds=hits, gpu_s_median=(ms_per_step * 1e-3 * (med + 1) / cfg.n_sweeps) if med is not None else None)
         tts["speedup_vs_oracle"] = (tts["cpu_s"] / tts["gpu_s"]) if tts["gpu_s"] else None
         kw.pop("energy_threshold")
+
+    # ---------------- global-only and local-only rates, short runs from the final states ----------
+    phase_rates = None
+    if rank == 0 and world == 1:
+        phase_rates = {}
+        cyc = cfg.n_global + cfg.n_local
+        for name, (ng, nl, sw) in (("global_only", (1, 0, max(2, 2 * cfg.n_global))), ("local_only", (0, 1, max(10, 2 * cfg.n_local)))):
+            pk = dict(kw, n_global=ng, n_local=nl, sweep_offset=cfg.n_sweeps)
+            tmp = states.clone()
+            g.run(tmp, 1, want=("energy",), **pk)
+            a2, b2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a2.record(stream); g.run(tmp, sw, want=("energy",), **pk); b2.record(stream)
+            torch.cuda.synchronize()
+            phase_rates[name] = dict(value=B * sw * n / (a2.elapsed_time(b2) * 1e-3), unit=UNIT, sweeps=sw,
+                                     ms_per_sweep=a2.elapsed_time(b2) / sw)
 
     # ---------------- e2e: the same step through amh_run_host, pinned host buffers ----------------
     e2e = None
@@ -384,7 +411,7 @@ def main():
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
                 data="synthetic", config=workload, clocks=clocks, e2e=e2e, gpu_launches=launches,
-                roofline=roofline, cpu_baseline=cpu_baseline, time_to_threshold=tts)
+                roofline=roofline, cpu_baseline=cpu_baseline, time_to_threshold=tts, phase_rates=phase_rates)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
