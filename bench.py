@@ -219,6 +219,7 @@ def main():
     ap.add_argument("--spec-local", type=int, default=0)
     ap.add_argument("--ring-cols", type=int, default=0)
     ap.add_argument("--lanes-per-step", type=int, default=0)
+    ap.add_argument("--exchange", action="store_true", help="configs with temperature replicas: amh_run_pt (replica exchange after every cycle, NEXT-3) instead of amh_run; the line says so")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -289,14 +290,30 @@ def main():
     stream = torch.cuda.current_stream()
     info = g.launch_info(B, cfg.window)
 
+    exchange = bool(args.exchange and cfg.replicas)
     tts = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not exchange:
         tts = oracle_threshold(cfg)
         kw["energy_threshold"] = tts["threshold"]
 
+    if exchange:
+        args.no_e2e = True                                   # the exchange run is an experiment line: device-timed rate only
+        # replica exchange: one amh_run per cycle + amh_exchange, enqueued by amh_run_pt; temperatures reset every step
+        T0 = kw.pop("per_chain_T")
+        Tcur = T0.clone()
+        ptkw = dict(n_global=cfg.n_global, n_local=cfg.n_local, window=cfg.window, seed=kw["seed"], chain_offset=chain_offset)
+        n_cycles = cfg.n_sweeps // (cfg.n_global + cfg.n_local)
+        workload["exchange"] = "amh_run_pt: %d cycles, exchange after each, groups of %d" % (n_cycles, cfg.replicas)
+
+    def run_step():
+        if exchange:
+            Tcur.copy_(T0)
+            return g.run_pt(states, n_cycles, Tcur, cfg.replicas, **ptkw)
+        return g.run(states, cfg.n_sweeps, want=("energy", "best_energy"), **kw)
+
     def one_step():
         states.copy_(s0_dev)
-        return g.run(states, cfg.n_sweeps, want=("energy", "best_energy"), **kw)
+        return run_step()
 
     for _ in range(args.warmup):
         one_step()
@@ -309,9 +326,9 @@ def main():
         flush.fill_(1)                                  # L2 flush between timed iterations (outside the events)
         states.copy_(s0_dev)
         a.record(stream)
-        res = g.run(states, cfg.n_sweeps, want=("energy", "best_energy"), **kw)
+        res = run_step()
         b.record(stream)
-        launches += 1
+        launches += (2 * n_cycles) if exchange else 1
     barrier()
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
     clocks = sampler.stop() if sampler else None
@@ -346,7 +363,7 @@ def main():
 
     # ---------------- global-only and local-only rates, short runs from the final states ----------
     phase_rates = None
-    if rank == 0 and world == 1:
+    if rank == 0 and world == 1 and not exchange:
         phase_rates = {}
         cyc = cfg.n_global + cfg.n_local
         for name, (ng, nl, sw) in (("global_only", (1, 0, max(2, 2 * cfg.n_global))), ("local_only", (0, 1, max(10, 2 * cfg.n_local)))):

@@ -165,6 +165,31 @@ amh_status amh_run(amh_ctx *ctx, float *states, long long B, long long n_sweeps,
                    const amh_proposal *prop, unsigned long long seed, const amh_outputs *out,
                    void *cuda_stream);
 
+/* NEXT-3, replica exchange (PAPER.md:160 names parallel tempering as the companion of multi-block runs; DESIGN.md
+ * R23).  Chains chain_offset + b are grouped by `replicas` consecutive ids (B and chain_offset multiples of
+ * replicas >= 2).  After cycle `cycle` the pairs (r, r+1) of every group with r = cycle (mod 2) are tested:
+ *     accept iff log u <= (1/T_a - 1/T_b) (V_a - V_b),  u = ((x0 >> 8) + 1) 2^-24,
+ *     x0 = word 0 of Philox(key = seed; counter = (cycle_lo, cycle_hi, chain id of r, 3)),
+ * in fp64 on the fp32 inputs; an accepted pair swaps its TEMPERATURES (states stay in their rows).
+ *   energies    DEVICE float [B]  current V of every chain (amh_run's `energy` output)
+ *   per_chain_T DEVICE float [B]  in/out
+ *   n_tried, n_accepted  DEVICE unsigned long long [1], incremented (not reset); NULL = not wanted */
+amh_status amh_exchange(amh_ctx *ctx, const float *energies, float *per_chain_T, long long B, int replicas,
+                        long long cycle, long long chain_offset, unsigned long long seed,
+                        unsigned long long *n_tried, unsigned long long *n_accepted, void *cuda_stream);
+
+/* Alternating MH with an exchange step after every cycle: n_cycles times { amh_run for one cycle
+ * (sched->n_global + sched->n_local sweeps, sweep_offset = cycle * that) at the chains' current temperatures;
+ * amh_exchange on the sweep-end energies }, all enqueued on the stream, nothing synchronised.
+ *   per_chain_T  DEVICE float [B], in/out (the temperatures each row holds at the end)
+ *   energy       DEVICE float [B], required: V of the final states (also the scratch the exchange reads)
+ *   best_energy  DEVICE float [B] or NULL: min over all sweep ends of the call
+ *   n_tried, n_accepted  DEVICE unsigned long long [1] or NULL; reset to 0 by the call */
+amh_status amh_run_pt(amh_ctx *ctx, float *states, long long B, long long n_cycles, long long cycle_offset,
+                      long long chain_offset, const amh_schedule *sched, float *per_chain_T, int replicas,
+                      const amh_proposal *prop, unsigned long long seed, float *energy, float *best_energy,
+                      unsigned long long *n_tried, unsigned long long *n_accepted, void *cuda_stream);
+
 /* The same call on HOST buffers: states, temp->per_chain_T and every pointer in *out are host memory.
  * Copies in, runs, copies out and synchronises the stream; device staging buffers are owned by the
  * context and grow on demand. */

@@ -10,6 +10,7 @@ for the passages of the paper each function follows and DESIGN.md for the readin
 from __future__ import annotations
 
 import ctypes as C
+import math
 import os
 import subprocess
 
@@ -225,3 +226,58 @@ class Model:
             d["per_chain_T"] = np.ascontiguousarray(d["per_chain_T"], dtype=np.float32)
         prm = self._params(**d)
         return float(lib().amho_temperature(C.byref(prm), C.c_longlong(t), C.c_longlong(row)))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# NEXT-3: replica exchange between the temperatures of a group (PAPER.md:160 names parallel tempering as the
+# companion of multi-block runs; BASELINE.json:12 gives config 4 eight temperature replicas).  DESIGN.md R23.
+# Plain numpy on top of Model.run; test infrastructure like everything else in this package.
+# ---------------------------------------------------------------------------------------------------------
+PURPOSE_SWAP = 3
+
+
+def exchange(energies, T, replicas: int, cycle: int, seed: int, chain_offset: int = 0):
+    """One exchange step after cycle `cycle` (R23).  Chains chain_offset + b are grouped by `replicas` consecutive
+    ids; the pairs (r, r+1) of a group with r = cycle (mod 2) are tested:
+        accept iff log u <= (1/T_a - 1/T_b) (V_a - V_b),   u = ((x0 >> 8) + 1) 2^-24  (R7),
+        x0 = word 0 of Philox(key = seed; counter = (cycle_lo, cycle_hi, chain id of r, 3)),
+    evaluated in fp64 on the fp32 energies and temperatures; an accepted pair swaps its TEMPERATURES (the states stay
+    in their rows).  Returns (new T fp32 [B], accept flags of the tested pairs as a dict row_a -> 0/1, gaps)."""
+    V = np.asarray(energies, dtype=np.float32).astype(np.float64)
+    Tn = np.array(T, dtype=np.float32, copy=True)
+    B = V.shape[0]
+    if replicas < 2 or B % replicas or chain_offset % replicas:
+        raise ValueError("exchange: B and chain_offset must be multiples of replicas >= 2")
+    acc, gap = {}, {}
+    for g0 in range(0, B, replicas):
+        for r in range(cycle % 2, replicas - 1, 2):
+            a, b = g0 + r, g0 + r + 1
+            chain = chain_offset + a
+            ctr = np.array([[cycle & 0xffffffff, (cycle >> 32) & 0xffffffff, chain & 0xffffffff, PURPOSE_SWAP]], np.uint32)
+            key = np.array([[seed & 0xffffffff, (seed >> 32) & 0xffffffff]], np.uint32)
+            x0 = int(np.asarray(philox4x32_10(ctr, key)).reshape(-1)[0])
+            lu = math.log(((x0 >> 8) + 1) * 2.0 ** -24)
+            d = (1.0 / float(Tn[a]) - 1.0 / float(Tn[b])) * (V[a] - V[b])
+            ok = lu <= d
+            acc[a], gap[a] = int(ok), lu - d
+            if ok:
+                Tn[a], Tn[b] = Tn[b], Tn[a]
+    return Tn, acc, gap
+
+
+def run_pt(model: "Model", states, n_cycles: int, T, replicas: int, *, n_global=1, n_local=2, window=8, seed=1,
+           chain_offset=0, cycle_offset=0, n_threads: int = 0, **run_kw):
+    """Alternating MH with an exchange step after every cycle: Model.run for one cycle at the chains' current
+    temperatures, then exchange() on the sweep-end energies.  Returns states, final T, energies, swap counts."""
+    s = np.array(states, dtype=np.float32, order="C")
+    Tn = np.array(T, dtype=np.float32, copy=True)
+    cyc = n_global + n_local
+    n_try = n_acc = 0
+    e = None
+    for y in range(cycle_offset, cycle_offset + n_cycles):
+        r = model.run(s, cyc, n_global=n_global, n_local=n_local, window=window, per_chain_T=Tn, seed=seed,
+                      chain_offset=chain_offset, sweep_offset=y * cyc, n_threads=n_threads, **run_kw)
+        s, e = r["states"], r["energy"]
+        Tn, acc, _ = exchange(e, Tn, replicas, y, seed, chain_offset)
+        n_try += len(acc); n_acc += sum(acc.values())
+    return dict(states=s, T=Tn, energy=e, n_swap_tried=n_try, n_swap_accepted=n_acc)

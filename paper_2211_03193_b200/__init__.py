@@ -24,7 +24,7 @@ PROP_UNIFORM, PROP_GRID, PROP_GAUSSIAN = 0, 1, 2
 
 # every symbol include/amh.h declares
 EXPORTS = ["amh_default_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
-           "amh_run", "amh_run_host", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
+           "amh_run", "amh_run_host", "amh_run_pt", "amh_exchange", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
            "amh_last_error", "amh_version"]
 
 
@@ -91,6 +91,11 @@ def lib():
                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_ulonglong, C.c_void_p, C.c_void_p]
         L.amh_run.argtypes = run_args
         L.amh_run_host.argtypes = run_args
+        L.amh_exchange.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_int, C.c_longlong, C.c_longlong,
+                                   C.c_ulonglong, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.amh_run_pt.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_longlong, C.c_longlong, C.c_longlong, C.c_void_p,
+                                 C.c_void_p, C.c_int, C.c_void_p, C.c_ulonglong, C.c_void_p, C.c_void_p, C.c_void_p,
+                                 C.c_void_p, C.c_void_p]
         L.amh_launch_info.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
         L.amh_launch_shape.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
         L.amh_philox_test.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]
@@ -272,6 +277,41 @@ class AMH:
                              C.byref(sc), C.byref(tp), C.byref(pr), int(seed), C.byref(o), _stream_ptr(stream)))
         r["_keepalive"] = pct
         return r
+
+    # ---- amh_exchange / amh_run_pt (NEXT-3) ---------------------------------------------------------
+    def exchange(self, energies, per_chain_T, replicas: int, cycle: int, seed: int = 1, chain_offset: int = 0, stream=None):
+        """amh_exchange: per_chain_T (cuda float32 [B]) is updated in place; returns (n_tried, n_accepted) device tensors."""
+        torch = _torch()
+        e = _dev(energies, torch.float32, "energies")
+        if not (isinstance(per_chain_T, torch.Tensor) and per_chain_T.is_cuda and per_chain_T.dtype == torch.float32
+                and per_chain_T.is_contiguous()):
+            raise ValueError("per_chain_T must be a contiguous cuda float32 tensor (it is updated in place)")
+        cnt = torch.zeros(2, dtype=torch.int64, device="cuda")
+        _check(lib().amh_exchange(self._h, e.data_ptr(), per_chain_T.data_ptr(), per_chain_T.numel(), int(replicas), int(cycle),
+                                  int(chain_offset), int(seed), cnt[0:1].data_ptr(), cnt[1:2].data_ptr(), _stream_ptr(stream)))
+        return cnt[0:1], cnt[1:2]
+
+    def run_pt(self, states, n_cycles: int, per_chain_T, replicas: int, *, n_global=1, n_local=2, window=8, global_first=True,
+               prop_mode=PROP_UNIFORM, grid=0, sigma_start=0.0, sigma_end=0.0, ramp_sigma=0, seed=1, chain_offset=0,
+               cycle_offset=0, stream=None):
+        """amh_run_pt on DEVICE tensors: states [B][n] and per_chain_T [B] (cuda float32) are updated in place."""
+        torch = _torch()
+        for t in (states, per_chain_T):
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+                raise ValueError("states and per_chain_T must be contiguous cuda float32 tensors (updated in place)")
+        s = states.view(-1, self.n)
+        B = s.shape[0]
+        if per_chain_T.numel() != B:
+            raise ValueError("per_chain_T must have B entries")
+        energy = torch.empty(B, dtype=torch.float32, device="cuda")
+        best = torch.empty(B, dtype=torch.float32, device="cuda")
+        cnt = torch.zeros(2, dtype=torch.int64, device="cuda")
+        sc, _, pr = self._structs(n_global, n_local, window, global_first, 1.0, 1.0, 0, None, prop_mode, grid,
+                                  sigma_start, sigma_end, ramp_sigma)
+        _check(lib().amh_run_pt(self._h, s.data_ptr(), B, int(n_cycles), int(cycle_offset), int(chain_offset), C.byref(sc),
+                                per_chain_T.data_ptr(), int(replicas), C.byref(pr), int(seed), energy.data_ptr(),
+                                best.data_ptr(), cnt[0:1].data_ptr(), cnt[1:2].data_ptr(), _stream_ptr(stream)))
+        return dict(energy=energy, best_energy=best, n_swap_tried=cnt[0:1], n_swap_accepted=cnt[1:2])
 
     def run_host(self, states: np.ndarray, n_sweeps: int, *, n_global=1, n_local=10, window=8, global_first=True,
                  t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,

@@ -510,6 +510,62 @@ amh_status amh_energy_host(amh_ctx *c, const float *states, long long B, float *
     return AMH_OK;
 }
 
+amh_status amh_exchange(amh_ctx *c, const float *energies, float *per_chain_T, long long B, int replicas, long long cycle,
+                        long long chain_offset, unsigned long long seed, unsigned long long *n_tried,
+                        unsigned long long *n_accepted, void *cuda_stream)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_exchange: ctx is NULL");
+    if (B < 0 || replicas < 2 || B % replicas || chain_offset % replicas || cycle < 0)
+        return fail(AMH_ERR_INVALID_ARG, "amh_exchange: B = %lld and chain_offset = %lld must be multiples of replicas = %d >= 2, cycle >= 0",
+                    B, chain_offset, replicas);
+    if (B == 0) return AMH_OK;
+    if (!energies || !per_chain_T) return fail(AMH_ERR_INVALID_ARG, "amh_exchange: energies / per_chain_T is NULL");
+    const long long pairs = (B / replicas) * (replicas / 2);
+    amh::exchange_kernel<<<(unsigned)((pairs + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(
+        energies, per_chain_T, B, replicas, cycle, seed, chain_offset, n_tried, n_accepted);
+    AMH_CUDA(cudaGetLastError());
+    return AMH_OK;
+}
+
+amh_status amh_run_pt(amh_ctx *c, float *states, long long B, long long n_cycles, long long cycle_offset,
+                      long long chain_offset, const amh_schedule *sc, float *per_chain_T, int replicas,
+                      const amh_proposal *pr, unsigned long long seed, float *energy, float *best_energy,
+                      unsigned long long *n_tried, unsigned long long *n_accepted, void *cuda_stream)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_run_pt: ctx is NULL");
+    if (!sc || !per_chain_T || !energy) return fail(AMH_ERR_INVALID_ARG, "amh_run_pt: schedule / per_chain_T / energy is NULL");
+    if (n_cycles < 0 || cycle_offset < 0) return fail(AMH_ERR_INVALID_ARG, "amh_run_pt: n_cycles / cycle_offset < 0");
+    if (replicas < 2 || B % replicas || chain_offset % replicas)
+        return fail(AMH_ERR_INVALID_ARG, "amh_run_pt: B and chain_offset must be multiples of replicas >= 2");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (n_tried) AMH_CUDA(cudaMemsetAsync(n_tried, 0, sizeof(unsigned long long), st));
+    if (n_accepted) AMH_CUDA(cudaMemsetAsync(n_accepted, 0, sizeof(unsigned long long), st));
+    const long long cyc = (long long)sc->n_global + sc->n_local;
+    // the per-cycle best energies land in the staging arena, then fold into best_energy
+    float *cycle_best = nullptr;
+    if (best_energy && B > 0) {
+        amh_status stt = ensure_stage(c, up256((size_t)B * 4));
+        if (stt != AMH_OK) return stt;
+        cycle_best = static_cast<float *>(c->stage);
+    }
+    amh_temperature tp;
+    tp.t_start = tp.t_end = 1.0; tp.ramp_sweeps = 0; tp.per_chain_T = per_chain_T;
+    for (long long y = cycle_offset; y < cycle_offset + n_cycles; ++y) {
+        amh_outputs o;
+        std::memset(&o, 0, sizeof o);
+        o.energy = energy; o.best_energy = cycle_best;
+        amh_status stt = amh_run(c, states, B, cyc, y * cyc, chain_offset, sc, &tp, pr, seed, &o, cuda_stream);
+        if (stt != AMH_OK) return stt;
+        if (cycle_best && B > 0) {
+            amh::min_into_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(best_energy, cycle_best, B, y == cycle_offset);
+            AMH_CUDA(cudaGetLastError());
+        }
+        stt = amh_exchange(c, energy, per_chain_T, B, replicas, y, chain_offset, seed, n_tried, n_accepted, cuda_stream);
+        if (stt != AMH_OK) return stt;
+    }
+    return AMH_OK;
+}
+
 amh_status amh_philox_test(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long count, void *cuda_stream)
 {
     if (count < 0 || (count > 0 && (!ctr || !key || !out))) return fail(AMH_ERR_INVALID_ARG, "amh_philox_test: bad arguments");

@@ -112,4 +112,36 @@ __global__ void __launch_bounds__(128) energy_kernel(DevModel m, const float *__
 }
 
 
+// ------------------------------------------------------------------------------------------------
+// NEXT-3  replica exchange (R23): one thread per tested pair (r, r+1) of a group of `replicas`
+// consecutive chains, r = cycle (mod 2).  accept iff log u <= (1/T_a - 1/T_b)(V_a - V_b), evaluated in fp64 on
+// the fp32 energies and temperatures; an accepted pair swaps its temperatures.  Pairs are disjoint: no races.
+// ------------------------------------------------------------------------------------------------
+__global__ void exchange_kernel(const float *__restrict__ V, float *__restrict__ T, long long B, int replicas,
+                                long long cycle, unsigned long long seed, long long chain_offset,
+                                unsigned long long *__restrict__ n_tried, unsigned long long *__restrict__ n_accepted)
+{
+    const int per_group = (replicas - 1 - (int)(cycle & 1) + 1) / 2;      // pairs tested in one group this cycle
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (per_group <= 0 || q >= (B / replicas) * per_group) return;
+    const long long g = q / per_group;
+    const int r = (int)(cycle & 1) + 2 * (int)(q - g * per_group);
+    const long long a = g * replicas + r, b = a + 1;
+    const uint32_t x0 = draw0(seed, (unsigned long long)(chain_offset + a), (unsigned long long)cycle, 3u /* SWAP */);
+    const double lu = log((double)((x0 >> 8) + 1u) * 5.9604644775390625e-08);
+    const float ta = T[a], tb = T[b];
+    const double d = (1.0 / (double)ta - 1.0 / (double)tb) * ((double)V[a] - (double)V[b]);
+    const bool ok = lu <= d;
+    if (ok) { T[a] = tb; T[b] = ta; }
+    if (n_tried) atomicAdd(n_tried, 1ull);
+    if (n_accepted && ok) atomicAdd(n_accepted, 1ull);
+}
+
+// the running minimum of the sweep-end energies over the cycles of amh_run_pt
+__global__ void min_into_kernel(float *__restrict__ dst, const float *__restrict__ src, long long count, int first)
+{
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < count) dst[q] = first ? src[q] : fminf(dst[q], src[q]);
+}
+
 }  // namespace amh

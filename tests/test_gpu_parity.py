@@ -263,6 +263,48 @@ def test_trajectory_parity_gaussian_proposals(amh, orc, torch, synth, gpu_model)
     assert np.all(np.abs(e - want) < 1e-5 * np.abs(want))
 
 
+def test_replica_exchange_parity(amh, orc, torch, synth, gpu_model):
+    # NEXT-3 (R23): (i) the swap decisions of amh_exchange against the oracle's rule on the same fp32 energies and
+    # temperatures, bit for bit, over many random inputs, both cycle parities, several group sizes; (ii) amh_run_pt
+    # end to end against the oracle's run_pt: same final states, same permutation of the temperatures.
+    rng = np.random.default_rng(5)
+    g = gpu_model(40, 1000)
+    for replicas, B, off in ((2, 64, 0), (8, 64, 16), (3, 63, 3), (5, 40, 10)):
+        for cycle in (0, 1, 6, 2**33 + 1):
+            V = (rng.normal(3000.0, 30.0, B)).astype(np.float32)
+            T = gi.per_chain_temperature(B, replicas, 0.1, 5.0, off)
+            T = T[rng.permutation(B)] if cycle == 6 else T          # also states whose temperatures are already shuffled
+            want, acc, gap = orc.exchange(V, T, replicas, cycle, 11, off)
+            Td = torch.from_numpy(T.copy()).cuda()
+            nt, na = g.exchange(torch.from_numpy(V).cuda(), Td, replicas, cycle, seed=11, chain_offset=off)
+            assert np.array_equal(Td.cpu().numpy(), want), (replicas, cycle)
+            assert int(nt.item()) == len(acc) and int(na.item()) == sum(acc.values())
+            if len(acc) >= 16:
+                assert 0 < sum(acc.values()) < len(acc)              # both outcomes occur: the comparison has power
+    # (ii) config 4's shape in small: 8 temperatures 0.1..5, cycles of 1 global + 2 local sweeps
+    L, B, cycles = 40, 32, 6
+    ref, p, edges, m = synth(L, 1000)
+    s0 = gi.initial_states(B, 2 * L, seed=4)
+    T0 = gi.per_chain_temperature(B, 8, 0.1, 5.0)
+    kw = dict(n_global=1, n_local=2, window=4, seed=17)
+    o = orc.run_pt(m, s0, cycles, T0, 8, **kw)
+    st = torch.from_numpy(s0.copy()).cuda(); Td = torch.from_numpy(T0.copy()).cuda()
+    r = g.run_pt(st, cycles, Td, 8, **kw)
+    assert o["n_swap_accepted"] > 0
+    assert np.array_equal(Td.cpu().numpy(), o["T"])
+    assert np.array_equal(st.cpu().numpy(), o["states"])
+    assert int(r["n_swap_tried"].item()) == o["n_swap_tried"] and int(r["n_swap_accepted"].item()) == o["n_swap_accepted"]
+    e = r["energy"].cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(e - o["energy"]) < 1e-5 * np.abs(o["energy"]))
+    assert np.all(r["best_energy"].cpu().numpy() <= r["energy"].cpu().numpy() + 1e-3)
+    # split runs compose: 4 cycles then 2 more from cycle_offset 4
+    st2 = torch.from_numpy(s0.copy()).cuda(); T2 = torch.from_numpy(T0.copy()).cuda()
+    g.run_pt(st2, 4, T2, 8, **kw); g.run_pt(st2, 2, T2, 8, cycle_offset=4, **kw)
+    assert torch.equal(st2, st) and torch.equal(T2, Td)
+    with pytest.raises(amh.AMHError):
+        g.exchange(r["energy"][:30], Td[:30].contiguous(), 8, 0)          # B not a multiple of the group size
+
+
 @pytest.mark.parametrize("L", [2, 3, 5])
 def test_tiny_chains_run(amh, orc, torch, synth, gpu_model, L):
     # degenerate sizes: L < min_sep + 1 has no pairs (every proposal accepted); window clamps at both ends

@@ -290,3 +290,48 @@ def test_gaussian_proposal_law_wrap_and_sigma_ramp(orc, synth):
     allacc = np.ones((B, n), np.uint8)
     f3 = m.follow(s0, n, allacc, sigma_start=0.3, sigma_end=0.3, forced_prop=forced[:, :n], **kw)
     assert np.array_equal(f3["states"], forced[:, :n]) and np.array_equal(f3["prop"], f["prop"][:, :n])
+
+
+def test_replica_exchange_keeps_each_temperature_boltzmann_L4(orc, synth):
+    # P9 (NEXT-3, R23): pairs of chains at T = 1 and T = 2.5 on the L = 4 grid system of P4, one global sweep per cycle,
+    # an exchange attempt after every cycle.  A correct swap rule leaves the product law invariant, so the state that
+    # holds temperature T at the end must follow the enumerated Boltzmann law of T - for both temperatures.  A wrong
+    # sign or a swapped energy difference in the rule would pull the T = 1 holder towards the T = 2.5 law.
+    L, G, n = 4, 4, 8
+    ref, p, edges, m = synth(L, 1000)
+    eff = [1, 2, 3, 4, 5, 6]
+    idx = np.stack(np.meshgrid(*[np.arange(G)] * 6, indexing="ij"), -1).reshape(-1, 6)
+    states = np.zeros((len(idx), n), np.float32)
+    states[:, 0] = _grid_value(1, G); states[:, 7] = _grid_value(2, G)
+    for q, v in enumerate(eff):
+        states[:, v] = _grid_value(idx[:, q], G)
+    V = m.energy(states)
+    B = 2 * 32768
+    T0 = np.tile(np.array([1.0, 2.5], np.float32), B // 2)
+    start = gi.grid_states(B, n, G, seed=13)
+    r = orc.run_pt(m, start, 30, T0, 2, n_global=1, n_local=0, window=0, seed=6, prop_mode=orc.PROP_GRID, grid=G)
+    assert 0.2 < r["n_swap_accepted"] / r["n_swap_tried"] < 1.0        # the rule is exercised in both directions
+    assert r["n_swap_tried"] == 15 * (B // 2)                          # pair (0, 1) is tested on even cycles only
+    assert sorted(np.unique(r["T"]).tolist()) == [1.0, 2.5]
+    assert np.all(np.sort(r["T"].reshape(-1, 2), axis=1) == np.array([1.0, 2.5], np.float32))   # a permutation per group
+    s = r["states"]
+    cell = np.zeros(B, np.int64)
+    for v in eff:
+        mm = np.rint((s[:, v].astype(np.float64) / math.pi * G + G) / 2).astype(np.int64)
+        cell = cell * G + mm
+    for T in (1.0, 2.5):
+        w = np.exp(-(V - V.min()) / T)
+        prob = w / w.sum()
+        sel = r["T"] == np.float32(T)
+        assert sel.sum() == B // 2
+        counts = np.bincount(cell[sel], minlength=len(idx))
+        pval, cells = _chi2_p(counts, prob * sel.sum())
+        assert pval > 0.01, (T, pval)
+    # the two laws differ enough for the test to have power: the T = 1 holders tested against the T = 2.5 law fail
+    w = np.exp(-(V - V.min()) / 2.5); prob = w / w.sum()
+    sel = r["T"] == np.float32(1.0)
+    assert _chi2_p(np.bincount(cell[sel], minlength=len(idx)), prob * sel.sum())[0] < 1e-6
+    # equal temperatures: every attempt is accepted (log u <= 0) and nothing observable changes
+    Te = np.ones(8, np.float32)
+    Tn, acc, gap = orc.exchange(np.arange(8, dtype=np.float32), Te, 4, 1, 3)
+    assert list(acc.keys()) == [1, 5] and list(acc.values()) == [1, 1] and np.array_equal(Tn, Te)   # odd cycle: pair (1, 2) of each group
