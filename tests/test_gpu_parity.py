@@ -321,6 +321,48 @@ def test_tiny_chains_run(amh, orc, torch, synth, gpu_model, L):
         assert np.all(chk["acc"] == 1)
 
 
+def test_large_chain_wide_window_and_size_limit(amh, orc, torch, synth):
+    # maximum sizes and degenerate windows: (i) L = 1024 (123 KB of shared memory per chain, no room for the ring):
+    # a short traced run replayed by the oracle; (ii) a window wider than the chain makes the local phase global
+    # (R12: V_local(w >= L-1) = V), on the ring-free path; (iii) a chain too long for shared memory is refused.
+    L = 1024
+    ref, p, edges, m = synth(L, 1000)
+    g = amh.AMH(p, edges)
+    info = g.launch_info(2, 8)
+    assert info["chains_per_cta"] == 1 and info["smem_bytes"] <= 232448
+    s0 = gi.initial_states(2, 2 * L, seed=8)
+    st = torch.from_numpy(s0.copy()).cuda()
+    steps = 96
+    kw = dict(n_global=0, n_local=1, window=8, seed=2)
+    r = g.run(st, 1, trace_steps=steps, **kw)
+    _follow_check(m, s0, r, steps, **kw)
+    e = r["energy"].cpu().numpy().astype(np.float64)
+    want = m.energy(st.cpu().numpy())
+    assert np.all(np.abs(e - want) < 1e-5 * np.abs(want))
+    kw = dict(n_global=1, n_local=0, window=0, seed=2)
+    st = torch.from_numpy(s0.copy()).cuda()
+    r = g.run(st, 1, trace_steps=40, **kw)
+    _follow_check(m, s0, r, 40, **kw)
+    g.close()
+    # (ii)
+    L2 = 40
+    ref, p2, edges2, m2 = synth(L2, 1000)
+    g2 = amh.AMH(p2, edges2)
+    s1 = gi.initial_states(6, 2 * L2, seed=9)
+    wide = dict(n_global=0, n_local=1, window=1000, seed=3)
+    glob = dict(n_global=1, n_local=0, window=0, seed=3)
+    a = torch.from_numpy(s1.copy()).cuda(); b = torch.from_numpy(s1.copy()).cuda()
+    ra = g2.run(a, 3, trace_steps=3 * 2 * L2, **wide); rb = g2.run(b, 3, trace_steps=3 * 2 * L2, **glob)
+    assert g2.launch_info(6, 1000)["ring_cols"] == 0
+    assert torch.equal(ra["trace_acc"], rb["trace_acc"]) and torch.equal(a, b)
+    assert np.abs(ra["trace_dE"].cpu().numpy() - rb["trace_dE"].cpu().numpy()).max() < 1e-9
+    _follow_check(m2, s1, ra, 3 * 2 * L2, **wide)
+    # (iii)
+    with pytest.raises(amh.AMHError) as ex:
+        amh.AMH(np.full((2500, 2500, 2), 0.5, np.float32), np.array([2.0, 12.0, 22.0], np.float32))
+    assert ex.value.status == 2
+
+
 def test_zero_sweeps_and_empty_batch(amh, torch, synth, gpu_model):
     L = 16
     g = gpu_model(L, 1000)
