@@ -153,17 +153,15 @@ __device__ __forceinline__ Rot rot_about(double ax, double ay, double az, double
     return R;
 }
 
-// bin index and fraction of R8's interpolation at squared distance d2.  d = sqrt(d2) by one reciprocal-square-root
-// and one Newton step: within 1 ulp of the correctly rounded root (the coordinates feeding d2
-// are themselves rounded to fp32), at 5 instructions instead of sqrtf()'s 9 with its special-case branch.  d2 = 0
-// (coincident atoms) is mapped to the first bin by the floor below.  Rows in the ring are plain E[0..nb-1]: the caller
-// forms E[b+1] - E[b] itself, the same fp32 subtraction the packed table did at create.
+// bin index and fraction of R8's interpolation at squared distance d2.  d = sqrt.approx.f32(d2): one MUFU instruction,
+// maximum relative error 2^-23 (PTX ISA), i.e. within 1 ulp of the correctly rounded root (the
+// coordinates feeding d2 are themselves rounded to fp32), instead of sqrtf()'s 9 instructions with its special-case
+// branch; d2 = 0 (coincident atoms) gives 0 and lands in the first bin.  Rows in the ring are plain E[0..nb-1]: the
+// caller forms E[b+1] - E[b] itself, the same fp32 subtraction the packed table did at create.
 __device__ __forceinline__ void lerp_coords(float d2, float c0, float inv_delta, float tmax, int nb, int &b, float &f)
 {
-    d2 = fmaxf(d2, 1e-30f);
-    const float r = rsqrtf(d2);
-    float d = d2 * r;
-    d = fmaf(0.5f * r, fmaf(-d, d, d2), d);
+    float d;
+    asm("sqrt.approx.f32 %0, %1;" : "=f"(d) : "f"(d2));
     float t = (d - c0) * inv_delta;
     t = fminf(fmaxf(t, 0.0f), tmax);
     b = min((int)t, nb - 2);
