@@ -133,6 +133,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.c0 = (float)(e0 + 0.5 * delta);
     m.inv_delta = (float)(1.0 / delta);
     m.tmax = (float)(n_bins - 1);
+    m.t0 = (float)(-(e0 + 0.5 * delta) / delta);
     {
         // smallest fp32 d^2 from which pair_energy()'s t is surely clamped to tmax: the last bin centre with a
         // relative margin far above the rounding of sqrtf, the subtraction and the scaling (all monotone in d^2)

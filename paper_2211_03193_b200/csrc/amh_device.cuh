@@ -32,6 +32,7 @@ struct DevModel {
     const float *Epl;
     int row_stride;
     float c0, inv_delta, tmax;       // first bin centre, 1/bin width, nb-1
+    float t0;                        // -c0 / bin width
     float dfar;                      // >= sqrt(far2)
     float far2;                      // d^2 >= far2  =>  the clamp of R8 applies: e_ij(d) = Elast
     // bond-frame recursion H_{i+1} = H_i * A * Mplus(theta2, psi_i) * W * Rx(phi_{i+1})

@@ -158,11 +158,11 @@ __device__ __forceinline__ Rot rot_about(double ax, double ay, double az, double
 // coordinates feeding d2 are themselves rounded to fp32), instead of sqrtf()'s 9 instructions with its special-case
 // branch; d2 = 0 (coincident atoms) gives 0 and lands in the first bin.  Rows in the ring are plain E[0..nb-1]: the
 // caller forms E[b+1] - E[b] itself, the same fp32 subtraction the packed table did at create.
-__device__ __forceinline__ void lerp_coords(float d2, float c0, float inv_delta, float tmax, int nb, int &b, float &f)
+__device__ __forceinline__ void lerp_coords(float d2, float t0, float inv_delta, float tmax, int nb, int &b, float &f)
 {
     float d;
     asm("sqrt.approx.f32 %0, %1;" : "=f"(d) : "f"(d2));
-    float t = (d - c0) * inv_delta;
+    float t = fmaf(d, inv_delta, t0);                        // (d - c0) / delta with t0 = -c0 / delta: one fma
     t = fminf(fmaxf(t, 0.0f), tmax);
     b = min((int)t, nb - 2);
     f = t - (float)b;
@@ -246,8 +246,8 @@ __device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSou
                 for (int u = 0; u < U; ++u) {
                     en0[u] = en1[u] = eo0[u] = eo1[u] = 0.0f;
                     if (near[u]) {
-                        lerp_coords(d2n[u], m.c0, m.inv_delta, m.tmax, m.nb, bn[u], fn[u]);
-                        lerp_coords(d2o[u], m.c0, m.inv_delta, m.tmax, m.nb, bo[u], fo[u]);
+                        lerp_coords(d2n[u], m.t0, m.inv_delta, m.tmax, m.nb, bn[u], fn[u]);
+                        lerp_coords(d2o[u], m.t0, m.inv_delta, m.tmax, m.nb, bo[u], fo[u]);
                         const float *rowp = colp + iu[u] * m.row_stride;
                         en0[u] = rowp[bn[u]]; en1[u] = rowp[bn[u] + 1];
                         eo0[u] = rowp[bo[u]]; eo1[u] = rowp[bo[u] + 1];
@@ -262,8 +262,8 @@ __device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSou
                 for (int u = 0; u < U; ++u) {
                     vn[u] = vo[u] = make_float2(0.0f, 0.0f);
                     if (near[u]) {
-                        lerp_coords(d2n[u], m.c0, m.inv_delta, m.tmax, m.nb, bn[u], fn[u]);
-                        lerp_coords(d2o[u], m.c0, m.inv_delta, m.tmax, m.nb, bo[u], fo[u]);
+                        lerp_coords(d2n[u], m.t0, m.inv_delta, m.tmax, m.nb, bn[u], fn[u]);
+                        lerp_coords(d2o[u], m.t0, m.inv_delta, m.tmax, m.nb, bo[u], fo[u]);
                         const float2 *rowp = m.Epk + (size_t)tri_row(iu[u], j, m.L) * m.nb;
                         vn[u] = __ldg(rowp + bn[u]); vo[u] = __ldg(rowp + bo[u]);
                     }
@@ -347,7 +347,7 @@ __device__ __forceinline__ double team_full_energy(const DevModel &m, const floa
                     if (far[u]) v[u] = __ldg(m.Elast + rb + j);
                     else {
                         int b;
-                        lerp_coords(d2[u], m.c0, m.inv_delta, m.tmax, m.nb, b, f[u]);
+                        lerp_coords(d2[u], m.t0, m.inv_delta, m.tmax, m.nb, b, f[u]);
                         g[u] = __ldg(m.Epk + (size_t)(rb + j) * m.nb + b);
                     }
                 }
