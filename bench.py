@@ -219,6 +219,7 @@ def main():
     ap.add_argument("--spec-local", type=int, default=0)
     ap.add_argument("--ring-cols", type=int, default=0)
     ap.add_argument("--lanes-per-step", type=int, default=0)
+    ap.add_argument("--spec-global", type=int, default=-1)
     ap.add_argument("--exchange", action="store_true", help="configs with temperature replicas: amh_run_pt (replica exchange after every cycle, NEXT-3) instead of amh_run; the line says so")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -278,7 +279,7 @@ def main():
     p = gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi)
     g = pkg.AMH(p, edges, pkg.default_options(warps_per_chain=args.warps_per_chain, chains_per_cta=args.chains_per_cta,
                                                spec_local=args.spec_local, ring_cols=args.ring_cols,
-                                               lanes_per_step=args.lanes_per_step))
+                                               lanes_per_step=args.lanes_per_step, spec_global=args.spec_global))
     del p
     chain_offset, s0_np, kw = shard(cfg, rank, world)
     s0_host = torch.from_numpy(s0_np).pin_memory()

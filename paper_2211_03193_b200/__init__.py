@@ -38,7 +38,7 @@ class Options(C.Structure):
     _fields_ = [(k, C.c_double) for k in (
         "len_n_ca", "len_ca_c", "len_c_n", "ang_n_ca_c", "ang_ca_c_n", "ang_c_n_ca", "omega",
         "cb_len", "cb_ang", "cb_dih", "eps")] + [("min_sep", C.c_int), ("warps_per_chain", C.c_int), ("spec_local", C.c_int),
-                                         ("lanes_per_step", C.c_int), ("chains_per_cta", C.c_int), ("ring_cols", C.c_int)]
+                                         ("lanes_per_step", C.c_int), ("spec_global", C.c_int), ("chains_per_cta", C.c_int), ("ring_cols", C.c_int)]
 
 
 class _Schedule(C.Structure):

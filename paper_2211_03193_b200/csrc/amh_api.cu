@@ -80,6 +80,7 @@ amh_status amh_default_options(amh_options *o)
     o->chains_per_cta = 0;
     o->ring_cols = 0;
     o->lanes_per_step = 0;
+    o->spec_global = -1;
     return AMH_OK;
 }
 
@@ -227,7 +228,8 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     cudaFree(bad_dev); bad_dev = nullptr;
     if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
     m.Epk = c->Epk; m.Elast = c->Elast; m.Epl = c->Epl;
-    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
     AMH_CUDA_C(cudaFuncSetAttribute(amh::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
 #undef AMH_CUDA_C
     *out = c;
@@ -336,7 +338,7 @@ amh_status amh_launch_info(amh_ctx *c, long long B, int window, int *threads_per
     if (n_sm) *n_sm = c->n_sm;
     if (ctas_per_sm) {
         int nb = 0;
-        AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::sweep_kernel, 32 * (sh.C * sh.W + 1), sh.smem));
+        AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::sweep_kernel<false>, 32 * (sh.C * sh.W + 1), sh.smem));
         *ctas_per_sm = nb;
     }
     return AMH_OK;
@@ -410,7 +412,11 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     a.spec_local = c->opt.spec_local;
     a.lanes_per_step = c->opt.lanes_per_step > 0 ? c->opt.lanes_per_step : 8;
     const long long ctas = (B + sh.C - 1) / sh.C;
-    amh::sweep_kernel<<<(unsigned)ctas, 32 * (sh.C * sh.W + 1), sh.smem, st>>>(c->m, a);
+    // global proposals: one warp per step, speculatively, when a team has few warps (the whole team on one step when it
+    // has many: a speculative pass of W steps wastes the ones after the first accept)
+    const bool sg = c->opt.spec_global >= 0 ? c->opt.spec_global != 0 : sh.W <= 2;
+    if (sg) amh::sweep_kernel<true><<<(unsigned)ctas, 32 * (sh.C * sh.W + 1), sh.smem, st>>>(c->m, a);
+    else amh::sweep_kernel<false><<<(unsigned)ctas, 32 * (sh.C * sh.W + 1), sh.smem, st>>>(c->m, a);
     AMH_CUDA(cudaGetLastError());
     return AMH_OK;
 }

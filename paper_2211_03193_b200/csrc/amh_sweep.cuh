@@ -4,8 +4,8 @@
 // barrier; one more warp (the last) is the PRODUCER that feeds the table ring by TMA bulk copies.
 // Chains are independent: teams never wait for one another except through the ring.
 //
-// Global sweeps (Eq. 1, 3a): the team evaluates one proposal at a time over its O(L^2/6) straddling
-// pairs.  A thread owns a column j: it turns CB_j itself and walks the rows i in blocks of 8; a block
+// Global sweeps (Eq. 1, 3a): O(L^2/6) straddling pairs per proposal, evaluated either by the whole team one
+// proposal at a time (SG = false) or speculatively like the local ones, one warp per step (SG = true).  A thread owns a column j: it turns CB_j itself and walks the rows i in blocks of 8; a block
 // whose bounding sphere is beyond the last bin centre for both positions of CB_j is skipped whole, pairs
 // clamped before and after are skipped one by one (their term is exactly 0), near pairs gather 8 bytes
 // from the packed table in L2, four rows' gathers in flight at a time.
@@ -365,6 +365,9 @@ __device__ __forceinline__ double team_full_energy(const DevModel &m, const floa
     return tot;
 }
 
+// SG: global proposals too are evaluated speculatively, one warp per step (two instantiations, so that neither
+// carries the other's pair loop in its register budget)
+template <bool SG>
 __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, RunArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -561,7 +564,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 }
                 team_bar(bar_id, nthreads);
             }
-            if (is_global) {
+            if (is_global && !SG) {
                 // ======== one proposal, evaluated by the whole team ========================================
                 const int bi = k - batch_start;
                 const int split = (k >> 1) + (k & 1);
@@ -613,8 +616,12 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 ++k;
             } else {
                 // ======== up to nspec proposals, group r evaluating step k + r against the current state ===
-                const int S = min(nspec, batch_end - k);
-                if (use_ring) {
+                // (a global sweep in speculative mode: the groups are whole warps and the pairs are all straddling ones)
+                const bool gp = SG && is_global;
+                const int gl_x = gp ? 32 : gl, gpw_x = gp ? 1 : gpw;
+                const int grp_x = gp ? 0 : grp, glane_x = gp ? lane : glane;
+                const int S = min(gp ? min(nwarps, kMaxSpec) : nspec, batch_end - k);
+                if (use_ring && !gp) {
                     // columns left of the window centre are dead for this chain; wait for the ones the pass needs
                     if (tid == 0) prog[slot] = q0 + (k >> 1);
                     const int need = min(L - 1, ((k + S - 1) >> 1) + a.window);
@@ -624,7 +631,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                         mbar_wait(&full_bar[seen_slot], seen_par);
                     }
                 }
-                const int r = warp * gpw + grp;
+                const int r = warp * gpw_x + grp_x;
                 const bool active = r < S;
                 const int kk = k + r, bi = kk - batch_start;
                 const bool inert = (kk == 0) || (kk == n - 1);
@@ -633,19 +640,21 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 if (active && !inert) {
                     const int c = kk >> 1, split = c + (kk & 1);
                     Rk = step_rot(kk, bi);
-                    const int ilo = max(0, c - a.window), jhi = min(L - 1, c + a.window);
-                    // ---- a4: in-window cross pairs (Eq. 3b) -------------------------------------------------
-                    if (use_ring) {
+                    const int ilo = gp ? 0 : max(0, c - a.window), jhi = gp ? L - 1 : min(L - 1, c + a.window);
+                    // ---- a4/a5: in-window cross pairs (Eq. 3b), or all of them (Eq. 3a) ------------------------
+                    if (gp) {
+                        dE = cross_pairs_dE<false, true>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, 0, split, L - 1, lane, 32);
+                    } else if (use_ring) {
                         rs.slot0 = slot_j0 + split;
                         if (rs.slot0 >= R) rs.slot0 %= R;
-                        dE = cross_pairs_dE<true, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane, gl);
+                        dE = cross_pairs_dE<true, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane_x, gl_x);
                     } else {
-                        dE = cross_pairs_dE<false, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane, gl);
+                        dE = cross_pairs_dE<false, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane_x, gl_x);
                     }
                 }
                 // ---- a6: reduction over the group's lanes (every lane of the warp takes part) ----------------
-                for (int d = gl >> 1; d > 0; d >>= 1) dE += __shfl_xor_sync(0xffffffffu, dE, d);
-                if (active && glane == 0) {
+                for (int d = gl_x >> 1; d > 0; d >>= 1) dE += __shfl_xor_sync(0xffffffffu, dE, d);
+                if (active && glane_x == 0) {
                     sp_dE[r] = dE;
                     sp_acc[r] = (b_lu[bi] <= -dE * invT) ? 1 : 0;   // Eq. 2a, R14
                     if (!inert) {
@@ -671,7 +680,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 if (rsel < S) {
                     // ---- a7: commit the accepted step --------------------------------------------------------
                     const int kc = k + rsel;
-                    ++acc_l;
+                    if (gp) ++acc_g; else ++acc_l;
                     if (tid == 0) s[kc] = b_sp[kc - batch_start];
                     if (kc != 0 && kc != n - 1) {
                         Rot Rc;
@@ -680,6 +689,10 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
 #pragma unroll
                         for (int q = 0; q < 3; ++q) Rc.t[q] = rot_s[12 * rsel + 9 + q];
                         commit(Rc, kc);
+                        if (gp) {
+                            team_bar(bar_id, nthreads);
+                            team_blocks(m, cb4, blk4, (kc >> 1) / kBlk, tid, nthreads);
+                        }
                     }
                 }
                 team_bar(bar_id, nthreads);

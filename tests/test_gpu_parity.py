@@ -153,17 +153,18 @@ def _follow_check(m, s0, r, steps, **kw):
     return dict(err=err, n_diff=int(diff.sum()), n_near=int(near.sum()), f=f, acc=acc)
 
 
-@pytest.mark.parametrize("wpc,spec,cpc,ring,gl", [(0, 0, 0, 0, 0), (1, 0, 1, 0, 32), (4, 1, 1, -1, 16), (4, 0, 3, 0, 8),
-                                                  (2, 0, 7, 0, 16), (8, 3, 1, 0, 8), (15, 0, 1, -1, 32), (3, 2, 5, 11, 16),
-                                                  (1, 0, 12, 12, 8), (2, 16, 2, 0, 8)])
-def test_trajectory_parity_config0_first_1000_steps(amh, orc, torch, synth, wpc, spec, cpc, ring, gl):
+@pytest.mark.parametrize("wpc,spec,cpc,ring,gl,sg", [(0, 0, 0, 0, 0, -1), (1, 0, 1, 0, 32, 1), (4, 1, 1, -1, 16, 0), (4, 0, 3, 0, 8, 1),
+                                                     (2, 0, 7, 0, 16, -1), (8, 3, 1, 0, 8, 1), (15, 0, 1, -1, 32, 0), (3, 2, 5, 11, 16, 1),
+                                                     (1, 0, 12, 12, 8, 0), (2, 16, 2, 0, 8, 0), (15, 0, 1, 0, 8, 1)])
+def test_trajectory_parity_config0_first_1000_steps(amh, orc, torch, synth, wpc, spec, cpc, ring, gl, sg):
     # every launch shape walks the same trajectory: warps per chain, how many local proposals are evaluated
     # per pass (spec = 1 is the plain sequential order of Alg. 1), chains per CTA, and whether the rows of
-    # the local phase come from the shared-memory ring (TMA) or straight from L2 (ring = -1)
+    # the local phase come from the shared-memory ring (TMA) or straight from L2 (ring = -1), lanes per local proposal,
+    # and whether global proposals are evaluated one warp per step speculatively (sg) or by the whole team
     c = gi.CONFIGS[0]
     ref, p, edges, m = synth(c.L, c.cfg_seed)
     g = amh.AMH(p, edges, amh.default_options(warps_per_chain=wpc, spec_local=spec, chains_per_cta=cpc, ring_cols=ring,
-                                              lanes_per_step=gl))
+                                              lanes_per_step=gl, spec_global=sg))
     info = g.launch_info(c.B, c.window)
     assert (info["ring_cols"] > 0) == (ring >= 0)
     s0 = gi.initial_states(c.B, c.n, seed=1)
@@ -173,8 +174,8 @@ def test_trajectory_parity_config0_first_1000_steps(amh, orc, torch, synth, wpc,
     r = g.run(st, 8, trace_steps=steps, **kw)
     chk = _follow_check(m, s0, r, steps, **kw)
     err = chk["err"]
-    print("cfg0 wpc=%d spec=%d cpc=%d ring=%d lanes=%d: |dE_gpu - dE_oracle| median %.2e  p99 %.2e  max %.2e; decisions differing %d, near-ties %d of %d"
-          % (wpc, spec, cpc, ring, gl, np.median(err), np.quantile(err, 0.99), err.max(), chk["n_diff"], chk["n_near"], err.size))
+    print("cfg0 wpc=%d spec=%d cpc=%d ring=%d lanes=%d sg=%d: |dE_gpu - dE_oracle| median %.2e  p99 %.2e  max %.2e; decisions differing %d, near-ties %d of %d"
+          % (wpc, spec, cpc, ring, gl, sg, np.median(err), np.quantile(err, 0.99), err.max(), chk["n_diff"], chk["n_near"], err.size))
     assert err.max() < 2e-3
     assert np.quantile(err, 0.99) < 3e-4
     # first 1000 steps = 128 global + 872 local proposals: both phases are exercised
