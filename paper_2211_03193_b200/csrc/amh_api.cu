@@ -228,8 +228,10 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     cudaFree(bad_dev); bad_dev = nullptr;
     if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
     m.Epk = c->Epk; m.Elast = c->Elast; m.Epl = c->Epl;
-    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
-    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
     AMH_CUDA_C(cudaFuncSetAttribute(amh::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
 #undef AMH_CUDA_C
     *out = c;
@@ -338,7 +340,7 @@ amh_status amh_launch_info(amh_ctx *c, long long B, int window, int *threads_per
     if (n_sm) *n_sm = c->n_sm;
     if (ctas_per_sm) {
         int nb = 0;
-        AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::sweep_kernel<false>, 32 * (sh.C * sh.W + 1), sh.smem));
+        AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::sweep_kernel<false, false>, 32 * (sh.C * sh.W + 1), sh.smem));
         *ctas_per_sm = nb;
     }
     return AMH_OK;
@@ -415,8 +417,11 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     // global proposals: one warp per step, speculatively, when a team has few warps (the whole team on one step when it
     // has many: a speculative pass of W steps wastes the ones after the first accept)
     const bool sg = c->opt.spec_global >= 0 ? c->opt.spec_global != 0 : sh.W <= 2;
-    if (sg) amh::sweep_kernel<true><<<(unsigned)ctas, 32 * (sh.C * sh.W + 1), sh.smem, st>>>(c->m, a);
-    else amh::sweep_kernel<false><<<(unsigned)ctas, 32 * (sh.C * sh.W + 1), sh.smem, st>>>(c->m, a);
+    const unsigned threads = 32 * (sh.C * sh.W + 1);
+    if (sg && sh.R > 0) amh::sweep_kernel<true, true><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
+    else if (sg) amh::sweep_kernel<true, false><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
+    else if (sh.R > 0) amh::sweep_kernel<false, true><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
+    else amh::sweep_kernel<false, false><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
     AMH_CUDA(cudaGetLastError());
     return AMH_OK;
 }

@@ -367,7 +367,8 @@ __device__ __forceinline__ double team_full_energy(const DevModel &m, const floa
 
 // SG: global proposals too are evaluated speculatively, one warp per step (two instantiations, so that neither
 // carries the other's pair loop in its register budget)
-template <bool SG>
+// RING: the local phase reads its rows from the shared-memory ring (a.ring_cols > 0) or gathers them from L2.
+template <bool SG, bool RING>
 __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, RunArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -379,7 +380,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     const int tid = warp * 32 + lane, nthreads = W * 32, nwarps = W;
     const int bar_id = 1 + slot;
     const int span = min(2 * a.window, L - 1);            // largest j - i of an in-window pair
-    const bool use_ring = R > 0;
+    constexpr bool use_ring = RING;
 
     unsigned long long *full_bar = reinterpret_cast<unsigned long long *>(smem_raw);                 // [R]
     volatile long long *prog = reinterpret_cast<volatile long long *>(smem_raw + 8 * (size_t)R);      // [16]
@@ -644,12 +645,12 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                     // ---- a4/a5: in-window cross pairs (Eq. 3b), or all of them (Eq. 3a) ------------------------
                     if (gp) {
                         dE = cross_pairs_dE<false, true>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, 0, split, L - 1, lane, 32);
-                    } else if (use_ring) {
-                        rs.slot0 = slot_j0 + split;
-                        if (rs.slot0 >= R) rs.slot0 %= R;
-                        dE = cross_pairs_dE<true, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane_x, gl_x);
                     } else {
-                        dE = cross_pairs_dE<false, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane_x, gl_x);
+                        if (RING) {
+                            rs.slot0 = slot_j0 + split;
+                            if (rs.slot0 >= R) rs.slot0 %= R;
+                        }
+                        dE = cross_pairs_dE<RING, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane_x, gl_x);
                     }
                 }
                 // ---- a6: reduction over the group's lanes (every lane of the warp takes part) ----------------
