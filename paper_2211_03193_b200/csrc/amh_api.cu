@@ -416,7 +416,8 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     const long long ctas = (B + sh.C - 1) / sh.C;
     // global proposals: one warp per step, speculatively, when a team has few warps (the whole team on one step when it
     // has many: a speculative pass of W steps wastes the ones after the first accept)
-    const bool sg = c->opt.spec_global >= 0 ? c->opt.spec_global != 0 : sh.W <= 2;
+    // (and when the batch leaves most SMs empty: the wasted steps cost nothing there, the shorter critical path helps)
+    const bool sg = c->opt.spec_global >= 0 ? c->opt.spec_global != 0 : (sh.W <= 2 || 2 * ctas <= c->n_sm);
     const unsigned threads = 32 * (sh.C * sh.W + 1);
     if (sg && sh.R > 0) amh::sweep_kernel<true, true><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
     else if (sg) amh::sweep_kernel<true, false><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
