@@ -413,7 +413,7 @@ def main():
     pair_evals = algorithmic_pair_evals(cfg)
     achieved = pair_evals * LANE_OPS_PER_PAIR / (ms_per_step * 1e-3) / 1e9
     roofline = dict(bound="alu", achieved=achieved, peak=peak, unit="Glane-op/s", frac=achieved / peak,
-                    traffic=profiled_traffic(cfg.name), kernel="amh::sweep_kernel",
+                    traffic=profiled_traffic(cfg.name), kernel="amh::sweep_kernel<SG, RING> (one of four variants, chosen per launch)",
                     pair_evals_per_launch=pair_evals, lane_ops_per_pair_eval=LANE_OPS_PER_PAIR,
                     pair_evals_per_s=pair_evals / (ms_per_step * 1e-3),
                     peak_source="derived: %d SMs x 128 fp32 lanes x %.0f MHz (clocks.max.sm)" % (info["n_sm"], sm_max_mhz),

@@ -155,6 +155,10 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.loc[3][2] = o.cb_len * std::sin(o.cb_ang) * std::sin(o.cb_dih);
     m.h0x = o.len_n_ca;
     m.inv_len_n_ca = 1.0 / o.len_n_ca; m.inv_len_ca_c = 1.0 / o.len_ca_c;
+    // the C-beta as a fixed combination of the residue's own backbone atoms (ideal geometry: C lies at loc[2] in the frame)
+    m.cbA = m.loc[3][0] - m.loc[3][1] * m.loc[2][0] / m.loc[2][1];
+    m.cbB = m.loc[3][1] / m.loc[2][1];
+    m.cbC = m.loc[3][2] / m.loc[2][1];
 
     if (!(o.lanes_per_step == 0 || o.lanes_per_step == 8 || o.lanes_per_step == 16 || o.lanes_per_step == 32)) {
         delete c;
@@ -164,10 +168,10 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
         delete c;
         return fail(AMH_ERR_INVALID_ARG, "amh_create: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxSpec);
     }
-    if (amh::sweep_smem_bytes(n_res, 1, 0, 0, 0) > (size_t)c->max_smem) {
+    if (amh::sweep_smem_bytes(n_res, 1, 0, 0, 0, 0) > (size_t)c->max_smem) {
         delete c;
         return fail(AMH_ERR_UNSUPPORTED, "amh_create: L = %d needs %zu B of shared memory per chain, device allows %d",
-                    n_res, amh::sweep_smem_bytes(n_res, 1, 0, 0, 0), c->max_smem);
+                    n_res, amh::sweep_smem_bytes(n_res, 1, 0, 0, 0, 0), c->max_smem);
     }
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -295,7 +299,7 @@ amh_status amh_coords(amh_ctx *c, const float *states, long long B, float *cb_ou
 }
 
 // Launch shape of amh_run: C chains per CTA, W warps per chain, R ring slots.
-struct SweepShape { int C, W, R, ring_rows; size_t smem; };
+struct SweepShape { int C, W, R, ring_rows, cb64; size_t smem; };
 
 static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
 {
@@ -310,12 +314,15 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
         if (c->opt.ring_cols > 0) return std::max(c->opt.ring_cols, w_eff + 3);
         return w_eff + 3 + amh::kMaxSpec / 2 + (C > 1 ? 4 : 0);    // + reach of a speculative pass + drift between teams
     };
-    auto fits = [&](int C, int, int R) { return amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride) <= budget; };
+    sh.cb64 = 1;
+    auto fits = [&](int C, int, int R) { return amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride, sh.cb64) <= budget; };
     // chains per CTA: spread the batch over the SMs (one CTA each) and keep as many teams resident as shared memory
     // allows; the ring is added only when it fits beside them (warps in flight are worth more than the ring)
     int C = c->opt.chains_per_cta;
     if (C <= 0) {
-        C = (int)std::min<long long>(8, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));
+        C = (int)std::min<long long>(7, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));    // 7 x 2 warps + producer
+        // the fp64 C-betas (24 L bytes per chain) are dropped before a chain is (they can be rebuilt from N, CA, C)
+        if (!fits(C, 0, 0)) sh.cb64 = 0;
         while (C > 1 && !fits(C, 0, 0)) --C;
     }
     int W = c->opt.warps_per_chain;
@@ -327,7 +334,8 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
     }
     sh.C = C; sh.W = W; sh.R = R;
     if (R == 0) sh.ring_rows = 0;
-    sh.smem = amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride);
+    if (sh.cb64 && !fits(C, W, 0)) sh.cb64 = 0;              // forced shapes
+    sh.smem = amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride, sh.cb64);
     return sh;
 }
 
@@ -410,7 +418,7 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     if (sh.smem > (size_t)c->max_smem)
         return fail(AMH_ERR_UNSUPPORTED, "amh_run: L = %d, window = %d, %d chains x %d warps need %zu B of shared memory, device allows %d",
                     c->m.L, sc->window, sh.C, sh.W, sh.smem, c->max_smem);
-    a.C = sh.C; a.W = sh.W; a.ring_cols = sh.R; a.ring_rows = sh.ring_rows;
+    a.C = sh.C; a.W = sh.W; a.ring_cols = sh.R; a.ring_rows = sh.ring_rows; a.cb64 = sh.cb64;
     a.spec_local = c->opt.spec_local;
     a.lanes_per_step = c->opt.lanes_per_step > 0 ? c->opt.lanes_per_step : 8;
     const long long ctas = (B + sh.C - 1) / sh.C;

@@ -42,6 +42,7 @@ struct DevModel {
     double loc[4][3];                // N, CA, C, CB in the residue's bond frame (origin CA, x along N->CA)
     double h0x;                      // H_0 = [I | (len_n_ca, 0, 0)]
     double inv_len_n_ca, inv_len_ca_c;   // 1 / length of the bonds the torsions turn about
+    double cbA, cbB, cbC;            // CB = CA + cbA ex + cbB (C - CA) + cbC ex x (C - CA), ex = (CA - N) / |CA - N|   (R3)
 };
 
 // ------------------------------------------------------------------------------------------------

@@ -44,6 +44,7 @@ struct RunArgs {
     int lanes_per_step;                  // lanes that share one local proposal: 32, 16 or 8
     int ring_cols;                       // R: slots of the table ring (> window + 2), 0 = gather from L2 instead
     int ring_rows;                       // rows per column: 2w - min_sep + 1
+    int cb64;                            // fp64 C-betas kept in shared memory (else rebuilt from N, CA, C)
     unsigned long long seed;
     float *energy, *best_energy, *best_state;
     unsigned long long *n_accept_local, *n_accept_global;
@@ -64,14 +65,16 @@ constexpr int kMaxChains = 15;           // chains per CTA (named barriers 1..15
 constexpr int kSweepMaxThreads = 512;    // 15 team warps + the producer: 128 registers per thread
 
 // shared memory of one chain, in bytes (a multiple of 16):
-//   double X[4L], Y[4L], Z[4L]   atoms, index atom * L + res (atom 0..3 = N, CA, C, CB)
+//   double X[aL], Y[aL], Z[aL]   atoms, index atom * L + res (atom 0..2 = N, CA, C; a = 3).  The C-beta is a fixed
+//                                combination of the three (cb_point); it is kept in fp64 too (atom 3, a = 4) when
+//                                that does not cost a resident chain (cb64), else rebuilt where needed
 //   double red[16], b_cd[64], b_sd[64], b_lu[64], rot_s[16][12], sp_dE[16]
 //   float4 cb4[L]                fp32 copy of the C-betas (what the pair loops read)
 //   float4 blk4[ceil(L/8)]       bounding spheres of 8-residue blocks (culling in the global phase)
 //   float  s[n], b_sp[64];  int sp_acc[16]
-__host__ __device__ inline size_t chain_smem_bytes(int L)
+__host__ __device__ inline size_t chain_smem_bytes(int L, int cb64)
 {
-    const size_t doubles = 12 * (size_t)L + kMaxWarps + 3 * kDrawBatch + 12 * kMaxSpec + kMaxSpec;
+    const size_t doubles = (cb64 ? 12 : 9) * (size_t)L + (cb64 ? 0 : (L & 1)) + kMaxWarps + 3 * kDrawBatch + 12 * kMaxSpec + kMaxSpec;   // (L & 1): cb4 on 16 bytes
     size_t floats = 4 * (size_t)L + 4 * (((size_t)L + kBlk - 1) / kBlk) + 2 * (size_t)L + kDrawBatch + kMaxSpec;
     floats = (floats + 3) & ~(size_t)3;
     return sizeof(double) * doubles + sizeof(float) * floats;
@@ -80,11 +83,11 @@ __host__ __device__ inline size_t chain_smem_bytes(int L)
 // header: ring barriers, progress words; then the ring; then the chains
 __host__ __device__ inline size_t sweep_header_bytes(int ring_cols) { return (8 * (size_t)ring_cols + 8 * 16 + 15) & ~(size_t)15; }
 
-__host__ __device__ inline size_t sweep_smem_bytes(int L, int C, int ring_cols, int ring_rows, int row_stride)
+__host__ __device__ inline size_t sweep_smem_bytes(int L, int C, int ring_cols, int ring_rows, int row_stride, int cb64)
 {
     size_t b = sweep_header_bytes(ring_cols) + sizeof(float) * (size_t)ring_cols * ring_rows * row_stride;
     b = (b + 15) & ~(size_t)15;
-    return b + (size_t)C * chain_smem_bytes(L);
+    return b + (size_t)C * chain_smem_bytes(L, cb64);
 }
 
 // ---- PTX: mbarrier, TMA bulk copy, named barriers ----------------------------------------------------
@@ -153,6 +156,18 @@ __device__ __forceinline__ Rot rot_about(double ax, double ay, double az, double
     return R;
 }
 
+// C-beta of residue `res` from its own N, CA, C (fp64): ideal geometry makes it a fixed combination of them (R3)
+__device__ __forceinline__ void cb_point(const DevModel &m, const double *X, const double *Y, const double *Z, int L, int res,
+                                         double &x, double &y, double &z)
+{
+    const double ax = X[L + res], ay = Y[L + res], az = Z[L + res];                                  // CA
+    const double ex = (ax - X[res]) * m.inv_len_n_ca, ey = (ay - Y[res]) * m.inv_len_n_ca, ez = (az - Z[res]) * m.inv_len_n_ca;
+    const double vx = X[2 * L + res] - ax, vy = Y[2 * L + res] - ay, vz = Z[2 * L + res] - az;        // C - CA
+    x = fma(m.cbC, fma(ey, vz, -ez * vy), fma(m.cbB, vx, fma(m.cbA, ex, ax)));
+    y = fma(m.cbC, fma(ez, vx, -ex * vz), fma(m.cbB, vy, fma(m.cbA, ey, ay)));
+    z = fma(m.cbC, fma(ex, vy, -ey * vx), fma(m.cbB, vz, fma(m.cbA, ez, az)));
+}
+
 // bin index and fraction of R8's interpolation at squared distance d2.  d = sqrt.approx.f32(d2): one MUFU instruction,
 // maximum relative error 2^-23 (PTX ISA), i.e. within 1 ulp of the correctly rounded root (the
 // coordinates feeding d2 are themselves rounded to fp32), instead of sqrtf()'s 9 instructions with its special-case
@@ -190,7 +205,7 @@ __device__ __forceinline__ int tri_row(int i, int j, int L) { return (i * (2 * L
 // i; when a round has fewer columns than threads, S threads share a column and take every S-th row.
 template <bool RING, bool CULL>
 __device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSource &rs, const float4 *cb4, const float4 *blk4,
-                                                 const double *Xcb, const double *Ycb, const double *Zcb, const Rot &R,
+                                                 const double *X, const double *Y, const double *Z, bool cb64, const Rot &R,
                                                  int ilo, int split, int jhi, int tid, int nthr)
 {
     const int nJ = jhi - split + 1;
@@ -204,8 +219,10 @@ __device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSou
             if (slice >= S) break;
         }
         const int j = split + c0 + col;
-        double x, y, z;
-        rot_apply(R, Xcb[j], Ycb[j], Zcb[j], x, y, z);
+        double x0, y0, z0, x, y, z;
+        if (cb64) { x0 = X[3 * m.L + j]; y0 = Y[3 * m.L + j]; z0 = Z[3 * m.L + j]; }
+        else cb_point(m, X, Y, Z, m.L, j, x0, y0, z0);
+        rot_apply(R, x0, y0, z0, x, y, z);
         const float xn = (float)x, yn = (float)y, zn = (float)z;
         const float4 o = cb4[j];
         const int i_end = min(split - 1, j - m.min_sep);
@@ -440,16 +457,17 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     if (slot >= nvalid) return;
 
     // ================= team: one chain =====================================================================
-    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L);
-    double *X = reinterpret_cast<double *>(cbase), *Y = X + 4 * L, *Z = Y + 4 * L;
-    double *red = Z + 4 * L, *b_cd = red + kMaxWarps, *b_sd = b_cd + kDrawBatch, *b_lu = b_sd + kDrawBatch;
+    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L, a.cb64);
+    const bool cb64 = a.cb64 != 0;
+    const int na = cb64 ? 4 : 3;                            // atoms per residue kept in fp64
+    double *X = reinterpret_cast<double *>(cbase), *Y = X + na * L, *Z = Y + na * L;
+    double *red = Z + na * L + (cb64 ? 0 : (L & 1)), *b_cd = red + kMaxWarps, *b_sd = b_cd + kDrawBatch, *b_lu = b_sd + kDrawBatch;
     double *rot_s = b_lu + kDrawBatch, *sp_dE = rot_s + 12 * kMaxSpec;
     float4 *cb4 = reinterpret_cast<float4 *>(sp_dE + kMaxSpec);
     float4 *blk4 = cb4 + L;
     float *s = reinterpret_cast<float *>(blk4 + (L + kBlk - 1) / kBlk);
     float *b_sp = s + n;
     int *sp_acc = reinterpret_cast<int *>(b_sp + kDrawBatch);
-    const double *Xcb = X + 3 * L, *Ycb = Y + 3 * L, *Zcb = Z + 3 * L;
 
     const long long row = row0 + slot;
     const unsigned long long chain = (unsigned long long)(a.chain_offset + row);
@@ -458,9 +476,8 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     team_bar(bar_id, nthreads);
     if (warp == 0)
         nerf_build_warp(m, s, lane, [&](int res, int at, double x, double y, double z) {
-            const int f = at * L + res;
-            X[f] = x; Y[f] = y; Z[f] = z;
             if (at == 3) cb4[res] = make_float4((float)x, (float)y, (float)z, 0.0f);
+            if (at < na) { const int f = at * L + res; X[f] = x; Y[f] = y; Z[f] = z; }
         });
     team_bar(bar_id, nthreads);
 
@@ -490,16 +507,25 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     // residues; psi_c moves the residues after c (R19)
     auto commit = [&](const Rot &R_, int k) {
         const int c = k >> 1;
+        // a thread takes a residue: turns those of its backbone atoms that move, then rebuilds its C-beta from them
+        for (int res = c + ((k & 1) ? 1 : 0) + tid; res < L; res += nthreads) {
 #pragma unroll
-        for (int at = 0; at < 4; ++at) {
-            const int r0 = ((k & 1) == 0 && at >= 2) ? c : c + 1;
-            for (int res = r0 + tid; res < L; res += nthreads) {
+            for (int at = 0; at < 3; ++at) {
+                if (res == c && at < 2) continue;            // phi_c: N_c and CA_c are the axis
                 const int f = at * L + res;
                 double x, y, z;
                 rot_apply(R_, X[f], Y[f], Z[f], x, y, z);
                 X[f] = x; Y[f] = y; Z[f] = z;
-                if (at == 3) cb4[res] = make_float4((float)x, (float)y, (float)z, 0.0f);
             }
+            double x, y, z;
+            if (cb64 && (res > c || (k & 1) == 0)) {         // the stored C-beta turns with its residue
+                const int f = 3 * L + res;
+                rot_apply(R_, X[f], Y[f], Z[f], x, y, z);
+                X[f] = x; Y[f] = y; Z[f] = z;
+            } else {
+                cb_point(m, X, Y, Z, L, res, x, y, z);
+            }
+            cb4[res] = make_float4((float)x, (float)y, (float)z, 0.0f);
         }
     };
 
@@ -582,7 +608,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
 #pragma unroll
                             for (int q = 0; q < 3; ++q) rot_s[9 + q] = Rk.t[q];
                         }
-                        acc = warp_sum(cross_pairs_dE<false, true>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, 0, split, L - 1, tid, nthreads));
+                        acc = warp_sum(cross_pairs_dE<false, true>(m, rs, cb4, blk4, X, Y, Z, cb64, Rk, 0, split, L - 1, tid, nthreads));
                     }
                     if (lane == 0) red[warp] = acc;
                     team_bar(bar_id, nthreads);
@@ -644,13 +670,13 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                     const int ilo = gp ? 0 : max(0, c - a.window), jhi = gp ? L - 1 : min(L - 1, c + a.window);
                     // ---- a4/a5: in-window cross pairs (Eq. 3b), or all of them (Eq. 3a) ------------------------
                     if (gp) {
-                        dE = cross_pairs_dE<false, true>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, 0, split, L - 1, lane, 32);
+                        dE = cross_pairs_dE<false, true>(m, rs, cb4, blk4, X, Y, Z, cb64, Rk, 0, split, L - 1, lane, 32);
                     } else {
                         if (RING) {
                             rs.slot0 = slot_j0 + split;
                             if (rs.slot0 >= R) rs.slot0 %= R;
                         }
-                        dE = cross_pairs_dE<RING, false>(m, rs, cb4, blk4, Xcb, Ycb, Zcb, Rk, ilo, split, jhi, glane_x, gl_x);
+                        dE = cross_pairs_dE<RING, false>(m, rs, cb4, blk4, X, Y, Z, cb64, Rk, ilo, split, jhi, glane_x, gl_x);
                     }
                 }
                 // ---- a6: reduction over the group's lanes (every lane of the warp takes part) ----------------
