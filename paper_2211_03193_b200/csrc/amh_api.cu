@@ -232,10 +232,10 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     cudaFree(bad_dev); bad_dev = nullptr;
     if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
     m.Epk = c->Epk; m.Elast = c->Elast; m.Epl = c->Epl;
-    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
-    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
-    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
-    AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+#define AMH_SMEM_ATTR(SG_, RING_, CB_) AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<SG_, RING_, CB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem))
+    AMH_SMEM_ATTR(false, false, false); AMH_SMEM_ATTR(false, false, true); AMH_SMEM_ATTR(false, true, false); AMH_SMEM_ATTR(false, true, true);
+    AMH_SMEM_ATTR(true, false, false); AMH_SMEM_ATTR(true, false, true); AMH_SMEM_ATTR(true, true, false); AMH_SMEM_ATTR(true, true, true);
+#undef AMH_SMEM_ATTR
     AMH_CUDA_C(cudaFuncSetAttribute(amh::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
 #undef AMH_CUDA_C
     *out = c;
@@ -348,7 +348,7 @@ amh_status amh_launch_info(amh_ctx *c, long long B, int window, int *threads_per
     if (n_sm) *n_sm = c->n_sm;
     if (ctas_per_sm) {
         int nb = 0;
-        AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::sweep_kernel<false, false>, 32 * (sh.C * sh.W + 1), sh.smem));
+        AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::sweep_kernel<false, false, false>, 32 * (sh.C * sh.W + 1), sh.smem));
         *ctas_per_sm = nb;
     }
     return AMH_OK;
@@ -427,10 +427,19 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     // (and when the batch leaves most SMs empty: the wasted steps cost nothing there, the shorter critical path helps)
     const bool sg = c->opt.spec_global >= 0 ? c->opt.spec_global != 0 : (sh.W <= 2 || 2 * ctas <= c->n_sm);
     const unsigned threads = 32 * (sh.C * sh.W + 1);
-    if (sg && sh.R > 0) amh::sweep_kernel<true, true><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
-    else if (sg) amh::sweep_kernel<true, false><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
-    else if (sh.R > 0) amh::sweep_kernel<false, true><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
-    else amh::sweep_kernel<false, false><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a);
+    const int variant = (sg ? 4 : 0) | (sh.R > 0 ? 2 : 0) | (sh.cb64 ? 1 : 0);
+#define AMH_LAUNCH(SG_, RING_, CB_) amh::sweep_kernel<SG_, RING_, CB_><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a)
+    switch (variant) {
+    case 0: AMH_LAUNCH(false, false, false); break;
+    case 1: AMH_LAUNCH(false, false, true); break;
+    case 2: AMH_LAUNCH(false, true, false); break;
+    case 3: AMH_LAUNCH(false, true, true); break;
+    case 4: AMH_LAUNCH(true, false, false); break;
+    case 5: AMH_LAUNCH(true, false, true); break;
+    case 6: AMH_LAUNCH(true, true, false); break;
+    default: AMH_LAUNCH(true, true, true); break;
+    }
+#undef AMH_LAUNCH
     AMH_CUDA(cudaGetLastError());
     return AMH_OK;
 }

@@ -385,7 +385,8 @@ __device__ __forceinline__ double team_full_energy(const DevModel &m, const floa
 // SG: global proposals too are evaluated speculatively, one warp per step (two instantiations, so that neither
 // carries the other's pair loop in its register budget)
 // RING: the local phase reads its rows from the shared-memory ring (a.ring_cols > 0) or gathers them from L2.
-template <bool SG, bool RING>
+// CB64: the fp64 C-betas are kept in shared memory (a.cb64) or rebuilt from N, CA, C.
+template <bool SG, bool RING, bool CB64>
 __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, RunArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -458,7 +459,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
 
     // ================= team: one chain =====================================================================
     unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L, a.cb64);
-    const bool cb64 = a.cb64 != 0;
+    constexpr bool cb64 = CB64;
     const int na = cb64 ? 4 : 3;                            // atoms per residue kept in fp64
     double *X = reinterpret_cast<double *>(cbase), *Y = X + na * L, *Z = Y + na * L;
     double *red = Z + na * L + (cb64 ? 0 : (L & 1)), *b_cd = red + kMaxWarps, *b_sd = b_cd + kDrawBatch, *b_lu = b_sd + kDrawBatch;
