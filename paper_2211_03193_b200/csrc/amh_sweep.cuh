@@ -382,7 +382,7 @@ __device__ __forceinline__ double team_full_energy(const DevModel &m, const floa
     return tot;
 }
 
-// SG: global proposals too are evaluated speculatively, one warp per step (two instantiations, so that neither
+// SG: global proposals too are evaluated speculatively, one warp per step (separate instantiations, so that neither
 // carries the other's pair loop in its register budget)
 // RING: the local phase reads its rows from the shared-memory ring (a.ring_cols > 0) or gathers them from L2.
 // CB64: the fp64 C-betas are kept in shared memory (a.cb64) or rebuilt from N, CA, C.
