@@ -51,16 +51,29 @@ typedef enum {
     AMH_PARAM_TR5 = 1          /* 5 variables per residue (trRosetta2): not built, AMH_ERR_UNSUPPORTED */
 } amh_param;
 
-/* Geometry and energy options.  amh_default_options() fills the values every config of
- * BASELINE.json uses (R2, R3, R9).  Lengths in Angstrom, angles in radians. */
+/* Geometry, energy and numerics options (the MODEL; nothing about the launch).  amh_default_options() fills the
+ * values every config of BASELINE.json uses (R2, R3, R9).  Lengths in Angstrom, angles in radians. */
 typedef struct {
     double len_n_ca, len_ca_c, len_c_n;          /* 1.458, 1.525, 1.329 */
     double ang_n_ca_c, ang_ca_c_n, ang_c_n_ca;   /* 111.2, 116.2, 121.7 degrees */
     double omega;                                /* pi (trans) */
     double cb_len, cb_ang, cb_dih;               /* |CA-CB| 1.522, angle N-CA-CB 1.927, dihedral C-N-CA-CB -2.143 */
     double eps;                                  /* 1e-8, added to p inside the log */
+    double guard_scale;                          /* exact-decision guard (R24): pair energies are
+                                                    summed in fp32; a proposal whose gap |log u + dE/T| is below
+                                                    guard_scale * G(L, window, extent) / T - G being the bound on the fp32
+                                                    error of dE - is re-evaluated in fp64 (coordinates, root, -log(p + eps),
+                                                    interpolation) before the decision is taken, so that every decision is
+                                                    the one fp64 arithmetic gives.  1 = default; 0 = off (fp32 decisions);
+                                                    a huge value sends every proposal through the fp64 path */
     int    min_sep;                              /* 3: pairs need j - i >= min_sep; >= 1 */
-    int    warps_per_chain;                      /* amh_run launch shape: 0 = choose from L and B; else 1..15 */
+    int    pad_;
+} amh_options;
+
+/* Launch shape of amh_run (kernel internals, not part of the model; every field 0 / -1 = let the library choose).
+ * Set with amh_set_launch_options(); the parity tests run many shapes and require the same trajectory from all. */
+typedef struct {
+    int    warps_per_chain;                      /* 0 = choose from L and B; else 1..15 */
     int    spec_local;                           /* local proposals evaluated per pass (results consumed in order up to the
                                                     first accept: same trajectory); 0 = as many as the team has lane groups,
                                                     at most 16 */
@@ -71,7 +84,7 @@ typedef struct {
                                                     chains_per_cta * warps_per_chain <= 15 */
     int    ring_cols;                            /* slots of the shared-memory table ring of the local phase: 0 = choose,
                                                     -1 = off (rows gathered from L2), else >= window + 3 */
-} amh_options;
+} amh_launch_options;
 
 /* Alg. 1 / Fig. 1, R10, R12. */
 typedef struct {
@@ -84,7 +97,9 @@ typedef struct {
 /* R13.  T_t = t_start * (t_end/t_start)^(t/(ramp_sweeps-1)) for absolute sweep index t, constant
  * within a sweep, clamped to t_end for t >= ramp_sweeps-1; t_start == t_end or ramp_sweeps <= 1 means
  * constant t_start.  per_chain_T (DEVICE float[B], or NULL) overrides the ramp with one constant
- * temperature per row (config 4's replicas).  All temperatures must be > 0. */
+ * temperature per row (config 4's replicas).  All temperatures must be > 0: t_start / t_end are checked
+ * (INVALID_ARG); per_chain_T is checked by amh_run_host (host memory) and NOT by amh_run (device memory: a check
+ * would synchronise) - a row with T <= 0 there makes that row's decisions undefined. */
 typedef struct {
     double t_start, t_end;
     long long ramp_sweeps;
@@ -118,11 +133,17 @@ typedef struct {
     int   trace_steps;                    /* the first trace_steps proposals of the call are traced per chain */
     float *trace_prop;                    /* [B][trace_steps] proposed value s'_k */
     double *trace_dE;                     /* [B][trace_steps] dE the decision used */
-    unsigned char *trace_acc;             /* [B][trace_steps] 1 = accepted */
+    unsigned char *trace_acc;             /* [B][trace_steps] bit 0 = accepted; bit 1 = the decision was taken by the
+                                                 fp64 path of the exact-decision guard (trace_dE is then the fp64 dE) */
 } amh_outputs;
 
 /* Fill *opt with the defaults above.  opt: host. */
 amh_status amh_default_options(amh_options *opt);
+amh_status amh_default_launch_options(amh_launch_options *opt);
+
+/* Force (parts of) the launch shape of later amh_run calls on this context; NULL restores the defaults.
+ * INVALID_ARG when a field is out of range.  Host. */
+amh_status amh_set_launch_options(amh_ctx *ctx, const amh_launch_options *opt);
 
 /* Build a context: validate, compute E = -log(p + eps) (Eq. 3a) into device memory.
  *   out         host; receives the context

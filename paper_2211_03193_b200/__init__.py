@@ -23,7 +23,7 @@ __all__ = ["AMH", "AMHError", "Options", "lib", "lib_path", "default_options", "
 PROP_UNIFORM, PROP_GRID, PROP_GAUSSIAN = 0, 1, 2
 
 # every symbol include/amh.h declares
-EXPORTS = ["amh_default_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
+EXPORTS = ["amh_default_options", "amh_default_launch_options", "amh_set_launch_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
            "amh_run", "amh_run_host", "amh_run_pt", "amh_exchange", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
            "amh_last_error", "amh_version"]
 
@@ -34,11 +34,35 @@ class AMHError(RuntimeError):
         self.status = status
 
 
-class Options(C.Structure):
+class _ModelOptions(C.Structure):          # amh_options
     _fields_ = [(k, C.c_double) for k in (
         "len_n_ca", "len_ca_c", "len_c_n", "ang_n_ca_c", "ang_ca_c_n", "ang_c_n_ca", "omega",
-        "cb_len", "cb_ang", "cb_dih", "eps")] + [("min_sep", C.c_int), ("warps_per_chain", C.c_int), ("spec_local", C.c_int),
-                                         ("lanes_per_step", C.c_int), ("spec_global", C.c_int), ("chains_per_cta", C.c_int), ("ring_cols", C.c_int)]
+        "cb_len", "cb_ang", "cb_dih", "eps", "guard_scale")] + [("min_sep", C.c_int), ("pad_", C.c_int)]
+
+
+class _LaunchOptions(C.Structure):         # amh_launch_options
+    _fields_ = [(k, C.c_int) for k in ("warps_per_chain", "spec_local", "lanes_per_step", "spec_global", "chains_per_cta", "ring_cols")]
+
+
+class Options:
+    """amh_options (the model) and amh_launch_options (the launch shape) side by side; attribute access goes to
+    whichever struct has the field."""
+
+    def __init__(self):
+        object.__setattr__(self, "model", _ModelOptions())
+        object.__setattr__(self, "launch", _LaunchOptions())
+
+    def __getattr__(self, k):
+        for st in (self.model, self.launch):
+            if k in dict(st._fields_):
+                return getattr(st, k)
+        raise AttributeError(k)
+
+    def __setattr__(self, k, v):
+        for st in (self.model, self.launch):
+            if k in dict(st._fields_):
+                return setattr(st, k, v)
+        raise AttributeError(k)
 
 
 class _Schedule(C.Structure):
@@ -99,7 +123,9 @@ def lib():
         L.amh_launch_info.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
         L.amh_launch_shape.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
         L.amh_philox_test.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]
-        L.amh_default_options.argtypes = [C.POINTER(Options)]
+        L.amh_default_options.argtypes = [C.POINTER(_ModelOptions)]
+        L.amh_default_launch_options.argtypes = [C.POINTER(_LaunchOptions)]
+        L.amh_set_launch_options.argtypes = [C.c_void_p, C.POINTER(_LaunchOptions)]
         _lib = L
     return _lib
 
@@ -111,7 +137,8 @@ def _check(st: int):
 
 def default_options(**over) -> Options:
     o = Options()
-    _check(lib().amh_default_options(C.byref(o)))
+    _check(lib().amh_default_options(C.byref(o.model)))
+    _check(lib().amh_default_launch_options(C.byref(o.launch)))
     for k, v in over.items():
         setattr(o, k, v)
     return o
@@ -170,7 +197,13 @@ class AMH:
         self.n = 2 * self.L
         self.options = options
         _check(lib().amh_create(C.byref(self._h), self.L, 0, dptr, e.ctypes.data, self.n_bins,
-                                C.byref(options) if options is not None else None, _stream_ptr(stream)))
+                                C.byref(options.model) if options is not None else None, _stream_ptr(stream)))
+        if options is not None:
+            try:
+                _check(lib().amh_set_launch_options(self._h, C.byref(options.launch)))
+            except AMHError:
+                self.close()
+                raise
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -15,7 +15,14 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libamh_b200.so")
 SOURCES = ["amh_api.cu"]
-DEPS = ["amh_api.cu", "amh_kernels.cuh", "amh_device.cuh", os.path.join("..", "..", "include", "amh.h")]
+PTXAS_LOG = os.path.join(CSRC, "ptxas_info.txt")        # registers / spills of the last build (git-ignored)
+
+
+def deps():
+    """Every file the library is built from: all of csrc/*.cu, csrc/*.cuh and the public header."""
+    import glob
+    return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))) + \
+        [os.path.join(HERE, "..", "include", "amh.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -37,7 +44,7 @@ def stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
+    return any(os.path.getmtime(d) > t for d in deps())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -50,7 +57,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
         if verbose:
             sys.stderr.write(r.stderr)
-        with open(os.path.join(CSRC, "ptxas_info.txt"), "w") as f:
+        with open(PTXAS_LOG, "w") as f:
             f.write("# " + " ".join(cmd) + "\n" + r.stderr)
         os.replace(tmp, LIB)
     return LIB

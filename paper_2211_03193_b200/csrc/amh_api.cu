@@ -49,15 +49,33 @@ amh::Xf mplus(double ang, double tor, double len)
 struct amh_ctx {
     amh::DevModel m;
     amh_options opt;
+    amh_launch_options lopt;
     float2 *Epk = nullptr;       // upper-triangle lerp table (see DevModel)
     float *Elast = nullptr;
     float *Epl = nullptr;        // the same E, plain rows padded to row_stride floats (TMA source)
+    float *P = nullptr;          // the probabilities themselves (fp64 path of the exact-decision guard)
     int device = 0, n_sm = 0, max_smem = 0;
     // staging for the *_host calls (grow-only)
     void *stage = nullptr;
     size_t stage_bytes = 0;
-    unsigned long long *first_hit_dev = nullptr;   // scratch for amh_run's first-hit reduction
 };
+
+static amh_status check_launch_options(const amh_launch_options &o)
+{
+    const int w = o.warps_per_chain;
+    if (w < 0 || w > amh::kMaxTeamWarps)
+        return fail(AMH_ERR_INVALID_ARG, "launch options: warps_per_chain = %d outside [0, %d]", w, amh::kMaxTeamWarps);
+    const int cc = o.chains_per_cta;
+    if (cc < 0 || cc > amh::kMaxChains)
+        return fail(AMH_ERR_INVALID_ARG, "launch options: chains_per_cta = %d outside [0, %d]", cc, amh::kMaxChains);
+    if (w > 0 && cc > 0 && w * cc > amh::kMaxTeamWarps)
+        return fail(AMH_ERR_INVALID_ARG, "launch options: warps_per_chain * chains_per_cta = %d > %d", w * cc, amh::kMaxTeamWarps);
+    if (!(o.lanes_per_step == 0 || o.lanes_per_step == 8 || o.lanes_per_step == 16 || o.lanes_per_step == 32))
+        return fail(AMH_ERR_INVALID_ARG, "launch options: lanes_per_step = %d not in {0, 8, 16, 32}", o.lanes_per_step);
+    if (o.spec_local < 0 || o.spec_local > amh::kMaxSpec)
+        return fail(AMH_ERR_INVALID_ARG, "launch options: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxSpec);
+    return AMH_OK;
+}
 
 extern "C" {
 
@@ -74,13 +92,33 @@ amh_status amh_default_options(amh_options *o)
     o->omega = M_PI;
     o->cb_len = 1.522; o->cb_ang = 1.927; o->cb_dih = -2.143;
     o->eps = 1e-8;
+    o->guard_scale = 1.0;
     o->min_sep = 3;
+    o->pad_ = 0;
+    return AMH_OK;
+}
+
+amh_status amh_default_launch_options(amh_launch_options *o)
+{
+    if (!o) return fail(AMH_ERR_INVALID_ARG, "amh_default_launch_options: opt is NULL");
     o->warps_per_chain = 0;
     o->spec_local = 0;
-    o->chains_per_cta = 0;
-    o->ring_cols = 0;
     o->lanes_per_step = 0;
     o->spec_global = -1;
+    o->chains_per_cta = 0;
+    o->ring_cols = 0;
+    return AMH_OK;
+}
+
+amh_status amh_set_launch_options(amh_ctx *c, const amh_launch_options *o)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_set_launch_options: ctx is NULL");
+    amh_launch_options d;
+    amh_default_launch_options(&d);
+    if (o) d = *o;
+    amh_status st = check_launch_options(d);
+    if (st != AMH_OK) return st;
+    c->lopt = d;
     return AMH_OK;
 }
 
@@ -99,16 +137,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     if (opt) o = *opt;
     if (o.min_sep < 1) return fail(AMH_ERR_INVALID_ARG, "amh_create: min_sep = %d < 1", o.min_sep);
     if (!(o.eps >= 0.0)) return fail(AMH_ERR_INVALID_ARG, "amh_create: eps < 0");
-    {
-        const int w = o.warps_per_chain;
-        if (w < 0 || w > amh::kMaxTeamWarps)
-            return fail(AMH_ERR_INVALID_ARG, "amh_create: warps_per_chain = %d outside [0, %d]", w, amh::kMaxTeamWarps);
-        const int cc = o.chains_per_cta;
-        if (cc < 0 || cc > amh::kMaxChains)
-            return fail(AMH_ERR_INVALID_ARG, "amh_create: chains_per_cta = %d outside [0, %d]", cc, amh::kMaxChains);
-        if (w > 0 && cc > 0 && w * cc > amh::kMaxTeamWarps)
-            return fail(AMH_ERR_INVALID_ARG, "amh_create: warps_per_chain * chains_per_cta = %d > %d", w * cc, amh::kMaxTeamWarps);
-    }
+    if (!(o.guard_scale >= 0.0)) return fail(AMH_ERR_INVALID_ARG, "amh_create: guard_scale < 0");
     for (int b = 0; b <= n_bins; ++b)
         if (!std::isfinite(bin_edges[b])) return fail(AMH_ERR_INVALID_ARG, "amh_create: bin edge %d is not finite", b);
     const double e0 = bin_edges[0], e1 = bin_edges[n_bins];
@@ -124,6 +153,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     amh_ctx *c = new (std::nothrow) amh_ctx;
     if (!c) return fail(AMH_ERR_OOM, "amh_create: host allocation failed");
     c->opt = o;
+    amh_default_launch_options(&c->lopt);
     cudaError_t e = cudaGetDevice(&c->device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device);
@@ -142,7 +172,9 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
         const double lim = c_last * (1.0 + 1e-5) + 1e-5 * delta;
         m.far2 = std::nextafter((float)(lim * lim), INFINITY);
         m.dfar = std::nextafter((float)std::sqrt((double)m.far2), INFINITY);
+        m.far2_d = c_last * c_last * (1.0 + 1e-9);
     }
+    m.c0_d = e0 + 0.5 * delta; m.delta_d = delta; m.eps_d = o.eps;
     m.A = mplus(o.ang_n_ca_c, 0.0, o.len_ca_c);
     m.W = mplus(o.ang_c_n_ca, o.omega, o.len_n_ca);
     m.c2 = std::cos(o.ang_ca_c_n); m.s2 = std::sin(o.ang_ca_c_n); m.l3 = o.len_c_n;
@@ -160,14 +192,6 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.cbB = m.loc[3][1] / m.loc[2][1];
     m.cbC = m.loc[3][2] / m.loc[2][1];
 
-    if (!(o.lanes_per_step == 0 || o.lanes_per_step == 8 || o.lanes_per_step == 16 || o.lanes_per_step == 32)) {
-        delete c;
-        return fail(AMH_ERR_INVALID_ARG, "amh_create: lanes_per_step = %d not in {0, 8, 16, 32}", o.lanes_per_step);
-    }
-    if (o.spec_local < 0 || o.spec_local > amh::kMaxSpec) {
-        delete c;
-        return fail(AMH_ERR_INVALID_ARG, "amh_create: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxSpec);
-    }
     if (amh::sweep_smem_bytes(n_res, 1, 0, 0, 0, 0) > (size_t)c->max_smem) {
         delete c;
         return fail(AMH_ERR_UNSUPPORTED, "amh_create: L = %d needs %zu B of shared memory per chain, device allows %d",
@@ -188,7 +212,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
         if (c->Epk) cudaFree(c->Epk);
         if (c->Elast) cudaFree(c->Elast);
         if (c->Epl) cudaFree(c->Epl);
-        if (c->first_hit_dev) cudaFree(c->first_hit_dev);
+        if (c->P) cudaFree(c->P);
         delete c;
     };
 #define AMH_CUDA_C(call)                                                                           \
@@ -210,8 +234,8 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     }
     AMH_CUDA_C(cudaMalloc(&c->Epl, sizeof(float) * n_rows * m.row_stride));
     AMH_CUDA_C(cudaMemsetAsync(c->Epl, 0, sizeof(float) * n_rows * m.row_stride, st));
+    AMH_CUDA_C(cudaMalloc(&c->P, sizeof(float) * n_rows * n_bins));
     AMH_CUDA_C(cudaMalloc(&bad_dev, sizeof(int)));
-    AMH_CUDA_C(cudaMalloc(&c->first_hit_dev, sizeof(unsigned long long)));
     AMH_CUDA_C(cudaMemsetAsync(bad_dev, 0, sizeof(int), st));
     const float *src = distogram;
     if (!on_device) {
@@ -222,7 +246,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     {
         const int threads = 256;
         const int blocks = (int)std::min<long long>((count + threads - 1) / threads, (long long)c->n_sm * 16);
-        amh::table_kernel<<<blocks, threads, 0, st>>>(src, c->Epk, c->Elast, c->Epl, m.row_stride, n_res, n_bins, o.eps, bad_dev);
+        amh::table_kernel<<<blocks, threads, 0, st>>>(src, c->Epk, c->Elast, c->Epl, c->P, m.row_stride, n_res, n_bins, o.eps, bad_dev);
         AMH_CUDA_C(cudaGetLastError());
     }
     int bad = 0;
@@ -231,7 +255,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     if (bad) { cleanup(); return fail(AMH_ERR_INVALID_ARG, "amh_create: the distogram holds a negative, NaN or infinite value"); }
     cudaFree(bad_dev); bad_dev = nullptr;
     if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
-    m.Epk = c->Epk; m.Elast = c->Elast; m.Epl = c->Epl;
+    m.Epk = c->Epk; m.Elast = c->Elast; m.Epl = c->Epl; m.P = c->P;
 #define AMH_SMEM_ATTR(SG_, RING_, CB_) AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<SG_, RING_, CB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem))
     AMH_SMEM_ATTR(false, false, false); AMH_SMEM_ATTR(false, false, true); AMH_SMEM_ATTR(false, true, false); AMH_SMEM_ATTR(false, true, true);
     AMH_SMEM_ATTR(true, false, false); AMH_SMEM_ATTR(true, false, true); AMH_SMEM_ATTR(true, true, false); AMH_SMEM_ATTR(true, true, true);
@@ -245,12 +269,12 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
 amh_status amh_destroy(amh_ctx *c)
 {
     if (!c) return AMH_OK;
-    cudaDeviceSynchronize();
+    // cudaFree waits for the work that still uses the allocation: no device-wide synchronisation of our own
     if (c->Epk) cudaFree(c->Epk);
     if (c->Elast) cudaFree(c->Elast);
     if (c->Epl) cudaFree(c->Epl);
+    if (c->P) cudaFree(c->P);
     if (c->stage) cudaFree(c->stage);
-    if (c->first_hit_dev) cudaFree(c->first_hit_dev);
     delete c;
     return AMH_OK;
 }
@@ -310,22 +334,22 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
     sh.ring_rows = std::max(0, span - c->m.min_sep + 1);
     const size_t budget = (size_t)c->max_smem;
     auto ring_for = [&](int C) -> int {                       // slots: the window's columns + prefetch + drift between teams
-        if (c->opt.ring_cols < 0 || sh.ring_rows == 0) return 0;
-        if (c->opt.ring_cols > 0) return std::max(c->opt.ring_cols, w_eff + 3);
+        if (c->lopt.ring_cols < 0 || sh.ring_rows == 0) return 0;
+        if (c->lopt.ring_cols > 0) return std::max(c->lopt.ring_cols, w_eff + 3);
         return w_eff + 3 + amh::kMaxSpec / 2 + (C > 1 ? 4 : 0);    // + reach of a speculative pass + drift between teams
     };
     sh.cb64 = 1;
     auto fits = [&](int C, int, int R) { return amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride, sh.cb64) <= budget; };
     // chains per CTA: spread the batch over the SMs (one CTA each) and keep as many teams resident as shared memory
     // allows; the ring is added only when it fits beside them (warps in flight are worth more than the ring)
-    int C = c->opt.chains_per_cta;
+    int C = c->lopt.chains_per_cta;
     if (C <= 0) {
         C = (int)std::min<long long>(7, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));    // 7 x 2 warps + producer
         // the fp64 C-betas (24 L bytes per chain) are dropped before a chain is (they can be rebuilt from N, CA, C)
         if (!fits(C, 0, 0)) sh.cb64 = 0;
         while (C > 1 && !fits(C, 0, 0)) --C;
     }
-    int W = c->opt.warps_per_chain;
+    int W = c->lopt.warps_per_chain;
     W = W > 0 ? std::max(1, std::min(W, amh::kMaxTeamWarps / C)) : std::max(1, std::min(amh::kMaxTeamWarps / C, 8));
     int R = ring_for(C);
     if (R > 0 && !fits(C, W, R)) {
@@ -405,6 +429,14 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     a.prop_mode = pr ? pr->mode : AMH_PROP_UNIFORM; a.grid = pr ? pr->grid : 0;
     a.sigma_start = pr ? pr->sigma_start : 0.0; a.sigma_end = pr ? pr->sigma_end : 0.0; a.ramp_sigma = pr ? pr->ramp_sweeps : 0;
     a.seed = seed;
+    {
+        // exact-decision guard (R24): bound on |dE_fp32 - dE_fp64| at coordinates up to 32 A, scaled in the kernel by
+        // the chain's extent / 32 A.  Measured maxima with a safety factor of about 4.
+        const double gs = c->opt.guard_scale;
+        const int w_eff = std::min(sc->window, std::max(c->m.L - 1, 0));
+        a.guard_global = gs * 2e-3 * std::sqrt(std::max(c->m.L, 64) / 64.0);
+        a.guard_local = gs * 1e-3 * std::sqrt((w_eff + 1) / 9.0);
+    }
     if (out) {
         a.energy = out->energy; a.best_energy = out->best_energy; a.best_state = out->best_state;
         a.n_accept_local = out->n_accept_local; a.n_accept_global = out->n_accept_global;
@@ -419,13 +451,13 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
         return fail(AMH_ERR_UNSUPPORTED, "amh_run: L = %d, window = %d, %d chains x %d warps need %zu B of shared memory, device allows %d",
                     c->m.L, sc->window, sh.C, sh.W, sh.smem, c->max_smem);
     a.C = sh.C; a.W = sh.W; a.ring_cols = sh.R; a.ring_rows = sh.ring_rows; a.cb64 = sh.cb64;
-    a.spec_local = c->opt.spec_local;
-    a.lanes_per_step = c->opt.lanes_per_step > 0 ? c->opt.lanes_per_step : 8;
+    a.spec_local = c->lopt.spec_local;
+    a.lanes_per_step = c->lopt.lanes_per_step > 0 ? c->lopt.lanes_per_step : 8;
     const long long ctas = (B + sh.C - 1) / sh.C;
     // global proposals: one warp per step, speculatively, when a team has few warps (the whole team on one step when it
     // has many: a speculative pass of W steps wastes the ones after the first accept)
     // (and when the batch leaves most SMs empty: the wasted steps cost nothing there, the shorter critical path helps)
-    const bool sg = c->opt.spec_global >= 0 ? c->opt.spec_global != 0 : (sh.W <= 2 || 2 * ctas <= c->n_sm);
+    const bool sg = c->lopt.spec_global >= 0 ? c->lopt.spec_global != 0 : (sh.W <= 2 || 2 * ctas <= c->n_sm);
     const unsigned threads = 32 * (sh.C * sh.W + 1);
     const int variant = (sg ? 4 : 0) | (sh.R > 0 ? 2 : 0) | (sh.cb64 ? 1 : 0);
 #define AMH_LAUNCH(SG_, RING_, CB_) amh::sweep_kernel<SG_, RING_, CB_><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a)
@@ -461,6 +493,10 @@ amh_status amh_run_host(amh_ctx *c, float *states, long long B, long long n_swee
 {
     amh_status stt = check_run(c, states, B, n_sweeps, sweep_offset, sc, tp, pr, out);
     if (stt != AMH_OK) return stt;
+    if (tp->per_chain_T)
+        for (long long q = 0; q < B; ++q)
+            if (!(tp->per_chain_T[q] > 0.0f) || !std::isfinite(tp->per_chain_T[q]))
+                return fail(AMH_ERR_INVALID_ARG, "amh_run_host: per_chain_T[%lld] = %g is not a finite temperature > 0", q, (double)tp->per_chain_T[q]);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t n = (size_t)c->m.n, b = (size_t)B;
     const size_t ts = out ? (size_t)out->trace_steps : 0;

@@ -27,10 +27,14 @@ struct DevModel {
     //   Elast[r]    = e_ij(d) for every d >= the last bin centre (the clamped value of R8)
     //   Epl[r][b]   = E[b], rows padded to row_stride floats (16-byte multiples whose bank offset differs from row
     //                 to row): what the TMA bulk copies stage into shared memory for the local phase
+    //   P[r][b]     = p_ij(b) as given (fp32): the fp64 path of the exact-decision guard takes -log(p + eps) itself
     const float2 *Epk;
     const float *Elast;
     const float *Epl;
+    const float *P;
     int row_stride;
+    double c0_d, delta_d, eps_d;     // first bin centre, bin width, eps in fp64 (fp64 path)
+    double far2_d;                   // squared distance from which the fp64 path is surely clamped (last centre + margin)
     float c0, inv_delta, tmax;       // first bin centre, 1/bin width, nb-1
     float t0;                        // -c0 / bin width
     float dfar;                      // >= sqrt(far2)
@@ -205,6 +209,19 @@ __device__ __forceinline__ float pair_energy(const float2 *__restrict__ row, flo
     const float f = t - (float)b;
     const float2 v = __ldg(row + b);              // { E[b], E[b+1] - E[b] }: one 8-byte gather per evaluation
     return fmaf(f, v.y, v.x);
+}
+
+// The same term in fp64 from the probabilities themselves (exact-decision guard, R24): E_b = -log((double)p_b + eps),
+// interpolation without fma contraction, as the plain definition reads.
+__device__ __forceinline__ double pair_energy_exact(const float *__restrict__ prow, double d, double c0, double delta, double eps, int nb)
+{
+    double t = (d - c0) / delta;
+    t = fmin(fmax(t, 0.0), (double)(nb - 1));
+    int b = (int)floor(t);
+    b = min(b, nb - 2);
+    const double f = t - (double)b;
+    const double e0 = -log((double)__ldg(prow + b) + eps), e1 = -log((double)__ldg(prow + b + 1) + eps);
+    return __dadd_rn(e0, __dmul_rn(f, __dadd_rn(e1, -e0)));
 }
 
 // row index of the pair i < j in the upper-triangle tables: tri(i, j) = tri_base(i) + j

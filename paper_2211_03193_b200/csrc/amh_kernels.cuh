@@ -10,7 +10,7 @@ namespace amh {
 // a0  E = -log(p + eps)   (Eq. 3a; BASELINE.json:7's 1e-8)
 // ------------------------------------------------------------------------------------------------
 __global__ void table_kernel(const float *__restrict__ p, float2 *__restrict__ Epk, float *__restrict__ Elast,
-                             float *__restrict__ Epl, int row_stride, int L, int nb, double eps, int *__restrict__ bad)
+                             float *__restrict__ Epl, float *__restrict__ P, int row_stride, int L, int nb, double eps, int *__restrict__ bad)
 {
     const long long count = (long long)L * L * nb;
     const long long stride = (long long)gridDim.x * blockDim.x;
@@ -28,6 +28,7 @@ __global__ void table_kernel(const float *__restrict__ p, float2 *__restrict__ E
         const long long r = tri_base(i, L) + j;
         Epk[r * nb + b] = make_float2(e0, de);
         Epl[r * row_stride + b] = e0;
+        P[r * nb + b] = v;
         if (b == nb - 2) Elast[r] = fmaf(1.0f, de, e0);              // the value pair_energy() returns at t = tmax
     }
     if (local_bad) atomicOr(bad, 1);

@@ -46,6 +46,7 @@ struct RunArgs {
     int ring_rows;                       // rows per column: 2w - min_sep + 1
     int cb64;                            // fp64 C-betas kept in shared memory (else rebuilt from N, CA, C)
     unsigned long long seed;
+    double guard_local, guard_global;    // exact-decision guard: bound on the fp32 error of dE at 32 A extent (0 = off)
     float *energy, *best_energy, *best_state;
     unsigned long long *n_accept_local, *n_accept_global;
     unsigned long long *first_hit;       // min over chains of the absolute sweep index; ~0ull = none
@@ -313,6 +314,72 @@ __device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSou
     return acc;
 }
 
+// ---- exact-decision guard (R24) --------------------------------------------------------------
+// dE of the proposal at variable k in fp64, every term from the fp64 atoms and from -log(p + eps) itself: this
+// thread's share of the sum over (i, j), ilo <= i < split <= j <= jhi, j - i >= min_sep, of e(new) - e(old).
+// Pairs beyond the last bin centre before and after contribute exactly 0 (R8's clamp) and are skipped.
+__device__ __noinline__ double exact_dE_partial(const DevModel &m, const double *X, const double *Y, const double *Z, int cb64,
+                                               int k, double cd, double sd, int ilo, int jhi, int tid, int nthr)
+{
+    const int L = m.L;
+    const int split = (k >> 1) + (k & 1);
+    const int nJ = jhi - split + 1, nI = split - ilo;
+    if (nJ <= 0 || nI <= 0) return 0.0;
+    const int fa = (k & 1) * L + (k >> 1), fb = fa + L;
+    const Rot R = rot_about(X[fa], Y[fa], Z[fa], X[fb], Y[fb], Z[fb], cd, sd, (k & 1) ? m.inv_len_ca_c : m.inv_len_n_ca);
+    double acc = 0.0;
+    for (int idx = tid; idx < nI * nJ; idx += nthr) {
+        const int ii = idx / nJ;
+        const int i = ilo + ii, j = split + (idx - ii * nJ);
+        if (j - i < m.min_sep) continue;
+        double xi, yi, zi, xo, yo, zo, xn, yn, zn;
+        if (cb64) {
+            xi = X[3 * L + i]; yi = Y[3 * L + i]; zi = Z[3 * L + i];
+            xo = X[3 * L + j]; yo = Y[3 * L + j]; zo = Z[3 * L + j];
+        } else {
+            cb_point(m, X, Y, Z, L, i, xi, yi, zi);
+            cb_point(m, X, Y, Z, L, j, xo, yo, zo);
+        }
+        rot_apply(R, xo, yo, zo, xn, yn, zn);
+        double dx = xi - xo, dy = yi - yo, dz = zi - zo;
+        const double d2o = dx * dx + dy * dy + dz * dz;
+        dx = xi - xn; dy = yi - yn; dz = zi - zn;
+        const double d2n = dx * dx + dy * dy + dz * dz;
+        if (d2o >= m.far2_d && d2n >= m.far2_d) continue;
+        const float *prow = m.P + (size_t)tri_row(i, j, L) * m.nb;
+        acc += pair_energy_exact(prow, sqrt(d2n), m.c0_d, m.delta_d, m.eps_d, m.nb)
+             - pair_energy_exact(prow, sqrt(d2o), m.c0_d, m.delta_d, m.eps_d, m.nb);
+    }
+    return acc;
+}
+
+// sum over the team's threads; every thread returns the total (two team barriers)
+__device__ __forceinline__ double team_sum(double v, double *red, int warp, int nwarps, int lane, int bar_id)
+{
+    v = warp_sum(v);
+    if (lane == 0) red[warp] = v;
+    team_bar(bar_id, nwarps * 32);
+    double tot = 0.0;
+    for (int w = 0; w < nwarps; ++w) tot += red[w];
+    team_bar(bar_id, nwarps * 32);
+    return tot;
+}
+
+// largest |coordinate| of the chain's C-betas (the fp32 rounding of a coordinate, hence the error bound of dE, scales with it)
+__device__ __forceinline__ float team_extent(const float4 *cb4, int L, double *red, int tid, int nthr, int warp, int nwarps, int lane, int bar_id)
+{
+    float e = 0.0f;
+    for (int i = tid; i < L; i += nthr) { const float4 c = cb4[i]; e = fmaxf(e, fmaxf(fabsf(c.x), fmaxf(fabsf(c.y), fabsf(c.z)))); }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) e = fmaxf(e, __shfl_xor_sync(0xffffffffu, e, d));
+    if (lane == 0) red[warp] = (double)e;
+    team_bar(bar_id, nwarps * 32);
+    double tot = 0.0;
+    for (int w = 0; w < nwarps; ++w) tot = fmax(tot, red[w]);
+    team_bar(bar_id, nwarps * 32);
+    return (float)tot;
+}
+
 // bounding spheres of the blocks [first, last] of kBlk consecutive C-betas: blk4[b] = {centre, ((dfar + radius)(1 + 1e-5))^2}
 __device__ __forceinline__ void team_blocks(const DevModel &m, const float4 *cb4, float4 *blk4, int first, int tid, int nthr)
 {
@@ -484,6 +551,8 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
 
     double best = INFINITY, e_end = 0.0;
     unsigned long long acc_l = 0, acc_g = 0;
+    // exact-decision guard: the bound on the fp32 error of dE grows with the size of the coordinates (their fp32 rounding)
+    double ext_scale = fmax(1.0, (double)team_extent(cb4, L, red, tid, nthreads, warp, nwarps, lane, bar_id) * (1.0 / 32.0));
     // local proposals are evaluated by groups of gl lanes, 32 / gl groups per warp
     const int gshift = a.lanes_per_step == 8 ? 3 : (a.lanes_per_step == 16 ? 4 : 5);
     const int gl = 1 << gshift, gpw = 32 >> gshift;
@@ -616,14 +685,22 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                     for (int w = 0; w < nwarps; ++w) dE += red[w];
                 }
                 // ---- a7: Metropolis test, accept iff log u <= -dE / T   (Eq. 1a, R14) ---------------------
-                const bool accept = b_lu[bi] <= -dE * invT;
+                // exact-decision guard (R24): a gap inside the fp32 error bound of dE is decided by the fp64 path
+                bool exact = false;
+                if (!inert && fabs(b_lu[bi] + dE * invT) < a.guard_global * ext_scale * invT) {
+                    team_bar(bar_id, nthreads);                      // every thread has read red[]
+                    dE = team_sum(exact_dE_partial(m, X, Y, Z, cb64 ? 1 : 0, k, b_cd[bi], b_sd[bi], 0, L - 1, tid, nthreads),
+                                  red, warp, nwarps, lane, bar_id);
+                    exact = true;
+                }
+                const bool accept = exact ? (b_lu[bi] <= -dE / T) : (b_lu[bi] <= -dE * invT);
                 if (tid == 0) {
                     const long long q = (t - a.sweep_offset) * n + k;
                     if (q < a.trace_steps) {
                         const size_t z = (size_t)row * a.trace_steps + q;
                         if (a.trace_prop) a.trace_prop[z] = b_sp[bi];
                         if (a.trace_dE) a.trace_dE[z] = dE;
-                        if (a.trace_acc) a.trace_acc[z] = accept ? 1 : 0;
+                        if (a.trace_acc) a.trace_acc[z] = (accept ? 1 : 0) | (exact ? 2 : 0);
                     }
                 }
                 if (accept) {
@@ -684,7 +761,9 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 for (int d = gl_x >> 1; d > 0; d >>= 1) dE += __shfl_xor_sync(0xffffffffu, dE, d);
                 if (active && glane_x == 0) {
                     sp_dE[r] = dE;
-                    sp_acc[r] = (b_lu[bi] <= -dE * invT) ? 1 : 0;   // Eq. 2a, R14
+                    const double gd = (gp ? a.guard_global : a.guard_local) * ext_scale * invT;
+                    // Eq. 2a, R14; 2 = the gap is inside the fp32 error bound of dE: decided below by the fp64 path (R24)
+                    sp_acc[r] = (!inert && fabs(b_lu[bi] + dE * invT) < gd) ? 2 : ((b_lu[bi] <= -dE * invT) ? 1 : 0);
                     if (!inert) {
 #pragma unroll
                         for (int q = 0; q < 9; ++q) rot_s[12 * r + q] = Rk.r[q];
@@ -694,7 +773,22 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 }
                 team_bar(bar_id, nthreads);
                 int rsel = 0;                                 // first accepted step of the pass
-                while (rsel < S && !sp_acc[rsel]) ++rsel;
+                bool any_exact = false;
+                while (rsel < S) {
+                    int f = sp_acc[rsel];                     // the same value in every thread of the team
+                    if (f == 2) {
+                        const int kx = k + rsel, bx = kx - batch_start, cx = kx >> 1;
+                        const double dx = team_sum(exact_dE_partial(m, X, Y, Z, cb64 ? 1 : 0, kx, b_cd[bx], b_sd[bx],
+                                                                    gp ? 0 : max(0, cx - a.window), gp ? L - 1 : min(L - 1, cx + a.window),
+                                                                    tid, nthreads), red, warp, nwarps, lane, bar_id);
+                        f = 2 | ((b_lu[bx] <= -dx / T) ? 1 : 0);
+                        if (tid == 0) { sp_dE[rsel] = dx; sp_acc[rsel] = f; }   // after team_sum's barriers: every thread has read the 2
+                        any_exact = true;
+                    }
+                    if (f & 1) break;
+                    ++rsel;
+                }
+                if (any_exact) team_bar(bar_id, nthreads);    // the rewritten entries are read by the tracing threads
                 const int nstand = (rsel < S) ? rsel + 1 : S; // steps whose result stands
                 if (tid < nstand) {
                     const long long q = (t - a.sweep_offset) * n + k + tid;
@@ -733,6 +827,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
         }
         // ---- a9: book-keeping at the sweep end ----------------------------------------------------
         e_end = team_full_energy(m, cb4, red, warp, nwarps, lane, bar_id);
+        ext_scale = fmax(1.0, (double)team_extent(cb4, L, red, tid, nthreads, warp, nwarps, lane, bar_id) * (1.0 / 32.0));
         if (e_end < best) {
             best = e_end;
             if (a.best_state)

@@ -71,7 +71,7 @@ def test_device_philox_matches_kat_and_oracle(amh, orc):
 @pytest.mark.parametrize("L", [1, 2, 3, 4, 33, 64, 128, 256, 600])
 def test_coords_parity(amh, orc, torch, synth, gpu_model, L):
     g = gpu_model(L)
-    s = states_for(L, 7, 6)
+    s = states_for(L, 7, 1003)                 # R22: >= 1,000 seeded random states + the all-180 chain + a helix
     cb, at = g.coords(torch.from_numpy(s).cuda(), atoms=True)
     cb, at = cb.cpu().numpy(), at.cpu().numpy()
     worst64 = worst32 = worstD = 0.0
@@ -84,13 +84,13 @@ def test_coords_parity(amh, orc, torch, synth, gpu_model, L):
         tol = 1e-4 + np.abs(CB) * 2.0 ** -24
         assert np.all(np.abs(cb[b] - CB) <= tol)
         worst32 = max(worst32, float((np.abs(cb[b] - CB) - np.abs(CB) * 2.0 ** -24).max()))
-        if L > 1:
+        if L > 1 and (b < 8 or b >= len(s) - 2):
             Dg = np.linalg.norm(at[b][:, None, 3] - at[b][None, :, 3], axis=-1)
             Do = np.linalg.norm(CB[:, None] - CB[None], axis=-1)
             worstD = max(worstD, float(np.abs(Dg - Do).max()))
     assert worst64 < 1e-9          # the fp64 scan agrees with the sequential fp64 NeRF far below the bar
     assert worstD < 1e-9
-    print("L=%d  max|atoms64 - oracle| = %.3g A, distance matrix %.3g A" % (L, worst64, worstD))
+    print("L=%d  %d states: max|atoms64 - oracle| = %.3g A, fp32 C-beta beyond its own ulp %.3g A, distance matrix %.3g A" % (L, len(s), worst64, worst32, worstD))
 
 
 @pytest.mark.parametrize("L,cfg_seed", [(1, 1000), (3, 1000), (4, 1000), (33, 1000), (64, 1000), (128, 1001),
@@ -98,7 +98,7 @@ def test_coords_parity(amh, orc, torch, synth, gpu_model, L):
 def test_energy_parity(amh, orc, torch, synth, gpu_model, L, cfg_seed):
     ref, p, edges, m = synth(L, cfg_seed)
     g = gpu_model(L, cfg_seed)
-    B = 1003 if L <= 128 else (300 if L == 256 else 40)
+    B = 1003                                   # R22: >= 1,000 seeded random states + the all-180 chain + a helix + the reference
     s = np.concatenate([states_for(L, 11, B), ref[None]])
     e = g.energy(torch.from_numpy(s).cuda()).cpu().numpy().astype(np.float64)
     want = m.energy(s)
@@ -139,9 +139,21 @@ def test_min_sep_option(amh, orc, torch, synth):
 
 
 # ---------------------------------------------------------------------------------------------
+def guard_bound(L, window, is_global, T=1.0):
+    """DESIGN.md R24: the bound G on |dE_fp32 - dE_fp64| the exact-decision guard assumes at coordinates up to 32 A
+    (the kernel scales it by the chain's extent / 32 A, so this is the SMALLEST bound it ever uses)."""
+    if is_global:
+        return 2e-3 * math.sqrt(max(L, 64) / 64.0)
+    return 1e-3 * math.sqrt((min(window, L - 1) + 1) / 9.0)
+
+
 def _follow_check(m, s0, r, steps, **kw):
-    """Follow-mode protocol: the oracle replays the GPU's decisions and checks its own."""
-    acc = r["trace_acc"].cpu().numpy()
+    """Follow-mode protocol: the oracle replays the GPU's decisions and checks its own.
+    trace_acc bit 0 = accepted, bit 1 = decided by the fp64 path of the exact-decision guard (R24): there the
+    traced dE must be the oracle's to fp64 rounding; everywhere else the fp32 dE must stay inside the guard's bound."""
+    bits = r["trace_acc"].cpu().numpy()
+    acc = bits & 1
+    exact = (bits & 2) != 0
     prop = r["trace_prop"].cpu().numpy()
     dE = r["trace_dE"].cpu().numpy()
     f = m.follow(s0, steps, acc, **kw)
@@ -150,7 +162,18 @@ def _follow_check(m, s0, r, steps, **kw):
     diff = acc != f["acc"]
     near = np.abs(f["g"]) < 1e-4
     assert np.all(near[diff]), "decisions may differ only at near-ties |g| < 1e-4: g = %s" % f["g"][diff]
-    return dict(err=err, n_diff=int(diff.sum()), n_near=int(near.sum()), f=f, acc=acc)
+    if exact.any():
+        assert err[exact].max() < 1e-8 * max(1.0, np.abs(f["dE"][exact]).max()), err[exact].max()
+    # the guard's own assumption, checked on every traced step that took the fp32 path: |dE_fp32 - dE_oracle| < G
+    L, n = m.L, m.n
+    ng, nl = kw.get("n_global", 1), kw.get("n_local", 10)
+    t = (kw.get("sweep_offset", 0) * n + np.arange(steps)) // n
+    r_ = t % (ng + nl)
+    is_g = (r_ < ng) if kw.get("global_first", True) else (r_ >= nl)
+    bound = np.where(is_g, guard_bound(L, 0, True), guard_bound(L, kw.get("window", 8), False))[None, :]
+    ok = exact | (err < bound)
+    assert ok.all(), "fp32 dE outside the guard's bound: %s (bound %s)" % (err[~ok], np.broadcast_to(bound, err.shape)[~ok])
+    return dict(err=err, n_diff=int(diff.sum()), n_near=int(near.sum()), f=f, acc=acc, exact=exact, is_global=is_g)
 
 
 @pytest.mark.parametrize("wpc,spec,cpc,ring,gl,sg", [(0, 0, 0, 0, 0, -1), (1, 0, 1, 0, 32, 1), (4, 1, 1, -1, 16, 0), (4, 0, 3, 0, 8, 1),
@@ -176,7 +199,6 @@ def test_trajectory_parity_config0_first_1000_steps(amh, orc, torch, synth, wpc,
     err = chk["err"]
     print("cfg0 wpc=%d spec=%d cpc=%d ring=%d lanes=%d sg=%d: |dE_gpu - dE_oracle| median %.2e  p99 %.2e  max %.2e; decisions differing %d, near-ties %d of %d"
           % (wpc, spec, cpc, ring, gl, sg, np.median(err), np.quantile(err, 0.99), err.max(), chk["n_diff"], chk["n_near"], err.size))
-    assert err.max() < 2e-3
     assert np.quantile(err, 0.99) < 3e-4
     # first 1000 steps = 128 global + 872 local proposals: both phases are exercised
     # the states the kernel returns are the ones the forced replay ends in
@@ -205,7 +227,6 @@ def test_trajectory_parity_pure_phases_and_temperatures(amh, orc, torch, synth, 
     kw = dict(n_global=n_global, n_local=n_local, window=5, seed=77, t_start=T, t_end=T, chain_offset=3)
     r = g.run(st, sweeps, trace_steps=steps, **kw)
     chk = _follow_check(m, s0, r, steps, **kw)
-    assert chk["err"].max() < 2e-3
     assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
     assert 0 < chk["acc"].mean() < 1
 
@@ -247,7 +268,7 @@ def test_trajectory_parity_gaussian_proposals(amh, orc, torch, synth, gpu_model)
               sigma_end=math.radians(4), ramp_sigma=sweeps, chain_offset=2)
     st = torch.from_numpy(s0.copy()).cuda()
     r = g.run(st, sweeps, trace_steps=steps, **kw)
-    acc = r["trace_acc"].cpu().numpy(); prop = r["trace_prop"].cpu().numpy(); dE = r["trace_dE"].cpu().numpy()
+    acc = r["trace_acc"].cpu().numpy() & 1; prop = r["trace_prop"].cpu().numpy(); dE = r["trace_dE"].cpu().numpy()
     f = m.follow(s0, steps, acc, forced_prop=prop, **kw)
     d = np.abs(prop.astype(np.float64) - f["prop"].astype(np.float64))
     d = np.minimum(d, np.abs(d - 2 * math.pi))
@@ -255,7 +276,8 @@ def test_trajectory_parity_gaussian_proposals(amh, orc, torch, synth, gpu_model)
     assert np.all((prop >= -np.float32(math.pi)) & (prop < np.float32(math.pi)))
     diff = acc != f["acc"]
     assert np.all(np.abs(f["g"][diff]) < 1e-4)
-    assert np.abs(dE - f["dE"]).max() < 2e-3
+    ex = (r["trace_acc"].cpu().numpy() & 2) != 0
+    assert np.abs(dE - f["dE"])[~ex].max() < guard_bound(L, 5, True)
     assert np.array_equal(st.cpu().numpy(), f["states"])
     # small steps are accepted far more often than uniform resampling: the accept/commit path is exercised
     assert acc.mean() > 0.3
@@ -355,7 +377,7 @@ def test_large_chain_wide_window_and_size_limit(amh, orc, torch, synth):
     a = torch.from_numpy(s1.copy()).cuda(); b = torch.from_numpy(s1.copy()).cuda()
     ra = g2.run(a, 3, trace_steps=3 * 2 * L2, **wide); rb = g2.run(b, 3, trace_steps=3 * 2 * L2, **glob)
     assert g2.launch_info(6, 1000)["ring_cols"] == 0
-    assert torch.equal(ra["trace_acc"], rb["trace_acc"]) and torch.equal(a, b)
+    assert torch.equal(ra["trace_acc"] & 1, rb["trace_acc"] & 1) and torch.equal(a, b)
     assert np.abs(ra["trace_dE"].cpu().numpy() - rb["trace_dE"].cpu().numpy()).max() < 1e-9
     _follow_check(m2, s1, ra, 3 * 2 * L2, **wide)
     # (iii)
@@ -456,7 +478,9 @@ def test_global_mh_boltzmann_on_device_L4(amh, orc, torch, synth, gpu_model):
     assert pval > 0.01, pval
 
 
-@pytest.mark.parametrize("cid,sweeps,rows", [(1, 11, (0, 517, 1023)), (2, 3, (0, 2049, 4095)), (4, 3, (5, 8191))])
+@pytest.mark.parametrize("cid,sweeps,rows", [(1, 11, (0, 146, 293, 439, 517, 731, 877, 1023)),
+                                             (2, 3, (0, 585, 1170, 2049, 2341, 2926, 3511, 4095)),
+                                             (4, 3, (5, 1170, 2340, 3511, 4681, 5851, 7021, 8191))])
 def test_sampled_parity_at_bench_size(amh, orc, torch, synth, gpu_model, cid, sweeps, rows):
     # BASELINE.json's configs at FULL width, in the launch shape bench.py times (chains per CTA, ring, lane groups
     # chosen by the library for that B and window), a short run: the traced trajectories of sampled chains are
@@ -483,40 +507,104 @@ def test_sampled_parity_at_bench_size(amh, orc, torch, synth, gpu_model, cid, sw
         kr = dict(kw, chain_offset=row)
         if "per_chain_T" in kr:
             kr["per_chain_T"] = kr["per_chain_T"][row:row + 1]
-        chk = _follow_check(m, s0[row:row + 1], rr, steps, **kr)
-        assert chk["err"].max() < 2e-3 * max(1.0, c.L / 128.0)
+        _follow_check(m, s0[row:row + 1], rr, steps, **kr)
 
 
-def test_config0_in_full_against_the_free_running_oracle(amh, orc, torch, synth, gpu_model):
-    # config 0 in full (32 chains x 2,200 sweeps = 281,600 proposals per chain), both sides free-running: a chain stays
-    # bit-identical to the oracle's until the first decision that falls inside the fp32 noise of dE (R20), so most
-    # chains must END bit-identical, and every chain's reported energy must be the energy of the state it returns.
-    # (Measured on B200: 29 of 32 identical, one more re-converged after a tie.)
+@pytest.mark.parametrize("cpc,wpc,sg", [(0, 0, -1), (3, 2, 1), (1, 4, 0)])
+def test_exact_path_is_the_oracle(amh, orc, torch, synth, cpc, wpc, sg):
+    # R24 with an unbounded guard: every proposal that moves an atom is decided by the fp64 path.  Its dE must be the
+    # oracle's to fp64 rounding and no decision may differ at all (the 1e-4 window is never needed).
+    c = gi.CONFIGS[0]
+    ref, p, edges, m = synth(c.L, c.cfg_seed)
+    g = amh.AMH(p, edges, amh.default_options(guard_scale=1e30, chains_per_cta=cpc, warps_per_chain=wpc, spec_global=sg))
+    s0 = gi.initial_states(c.B, c.n, seed=3)
+    st = torch.from_numpy(s0.copy()).cuda()
+    steps = 4 * c.n
+    kw = dict(n_global=1, n_local=2, window=c.window, seed=9)
+    r = g.run(st, 4, trace_steps=steps, **kw)
+    chk = _follow_check(m, s0, r, steps, **kw)
+    kk = np.arange(steps) % c.n
+    inert = (kk == 0) | (kk == c.n - 1)
+    assert chk["exact"][:, ~inert].all() and not chk["exact"][:, inert].any()
+    assert chk["n_diff"] == 0
+    assert chk["err"].max() < 1e-9
+    assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+    free = m.run(s0, 4, **kw)
+    assert np.array_equal(free["states"], st.cpu().numpy())
+
+
+def test_guard_off_is_fp32(amh, orc, torch, synth):
+    # guard_scale = 0: no proposal goes through the fp64 path (the round-1 behaviour); decisions are still the oracle's
+    # wherever its gap is larger than the fp32 error
+    c = gi.CONFIGS[0]
+    ref, p, edges, m = synth(c.L, c.cfg_seed)
+    g = amh.AMH(p, edges, amh.default_options(guard_scale=0.0))
+    s0 = gi.initial_states(c.B, c.n, seed=3)
+    st = torch.from_numpy(s0.copy()).cuda()
+    steps = 4 * c.n
+    kw = dict(n_global=1, n_local=2, window=c.window, seed=9)
+    r = g.run(st, 4, trace_steps=steps, **kw)
+    bits = r["trace_acc"].cpu().numpy()
+    assert not (bits & 2).any()
+    f = m.follow(s0, steps, bits & 1, **kw)
+    diff = (bits & 1) != f["acc"]
+    assert np.all(np.abs(f["g"][diff]) < guard_bound(c.L, c.window, True))
+
+
+def test_config0_in_full_follow_mode(amh, orc, torch, synth, gpu_model):
+    # config 0 IN FULL (32 chains x 2,200 sweeps x 128 = 281,600 proposals per chain) replayed by the oracle in follow
+    # mode: proposals bit-identical, every decision the oracle's except where its own gap is |g| < 1e-4 (logged), the
+    # fp32 dE inside the guard's bound at every step, the fp64 dE of the guarded steps equal to the oracle's
     import bench
     c = gi.CONFIGS[0]
     ref, p, edges, m = synth(c.L, c.cfg_seed)
     g = gpu_model(c.L, c.cfg_seed)
     s0 = gi.initial_states(c.B, c.n, seed=1)
     kw = bench.run_kwargs(c, c.B, 0)
-    o = m.run(s0, c.n_sweeps, **kw)
+    steps = c.n_sweeps * c.n
     st = torch.from_numpy(s0.copy()).cuda()
-    r = g.run(st, c.n_sweeps, **kw)
-    s = st.cpu().numpy()
-    same = np.all(s == o["states"], axis=1)
-    assert same.sum() >= 24, same.sum()
-    assert np.array_equal(r["n_accept_global"].cpu().numpy()[same], o["n_accept_global"][same])
-    assert np.abs(r["n_accept_local"].cpu().numpy()[same].astype(np.int64) - o["n_accept_local"][same].astype(np.int64)).max() <= 2
-    e = r["energy"].cpu().numpy().astype(np.float64)
-    want = m.energy(s)
-    assert np.all(np.abs(e - want) < 1e-5 * np.abs(want))
-    be = r["best_energy"].cpu().numpy().astype(np.float64)
-    assert np.all(np.abs(be[same] - o["best_energy"][same]) < 1e-5 * np.abs(o["best_energy"][same]))
-    assert np.all(be <= e + 1e-3)
-    # the best states reproduce the best energies
-    bs = m.energy(r["best_state"].cpu().numpy())
-    assert np.all(np.abs(bs - be) < 1e-5 * np.abs(bs))
-    # the population as a whole reaches the same energies
-    assert abs(be.mean() - o["best_energy"].mean()) < 0.01 * abs(o["best_energy"].mean())
+    r = g.run(st, c.n_sweeps, trace_steps=steps, **kw)
+    chk = _follow_check(m, s0, r, steps, **kw)
+    err, ex = chk["err"], chk["exact"]
+    gaps = np.abs(chk["f"]["g"])
+    print("cfg0 in full, follow mode: %d steps; decisions differing %d (all at |g| < 1e-4), oracle near-ties %d; steps decided by the fp64 path %d "
+          "(%.3g %%), their max |dE - oracle| %.2e; fp32 steps: |dE - oracle| median %.2e p99 %.2e max %.2e (global) %.2e (local); smallest oracle gap "
+          "among fp32-decided steps %.2e"
+          % (err.size, chk["n_diff"], chk["n_near"], ex.sum(), 100.0 * ex.mean(), err[ex].max() if ex.any() else 0.0, np.median(err[~ex]),
+             np.quantile(err[~ex], 0.99), err[~ex & chk["is_global"][None, :]].max(), err[~ex & ~chk["is_global"][None, :]].max(),
+             gaps[~ex & (np.arange(steps) % c.n != 0)[None, :] & (np.arange(steps) % c.n != c.n - 1)[None, :]].min()))
+    assert chk["n_diff"] == 0                      # with the guard no decision is left to the 1e-4 window
+    assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+    # and so the FREE-running oracle ends in the same states, bit for bit, in every chain
+    o = m.run(s0, c.n_sweeps, **kw)
+    assert np.array_equal(o["states"], st.cpu().numpy())
+    assert np.array_equal(o["n_accept_local"], r["n_accept_local"].cpu().numpy())
+    assert np.array_equal(o["n_accept_global"], r["n_accept_global"].cpu().numpy())
+    assert np.array_equal(o["best_state"], r["best_state"].cpu().numpy())
+
+
+def test_cold_end_of_config2_ramp(amh, orc, torch, synth, gpu_model):
+    # config 2 at the COLD end of its 10 -> 0.1 ramp, where 1/T = 10 magnifies every error of dE: full width, launch shape
+    # of the bench; 110 sweeps from sweep 19,800 relax the random start, then three traced sweeps from 19,910 (a global
+    # sweep first: 19,910 = 11 x 1,810) are replayed by the oracle for 8 sampled chains
+    import bench
+    c = gi.CONFIGS[2]
+    ref, p, edges, m = synth(c.L, c.cfg_seed)
+    g = gpu_model(c.L, c.cfg_seed)
+    st = torch.from_numpy(gi.initial_states(c.B, c.n, seed=1)).cuda()
+    kw = bench.run_kwargs(c, c.B, 0)
+    g.run(st, 110, sweep_offset=19800, want=(), **kw)
+    s1 = st.cpu().numpy().copy()
+    steps = 2 * c.n
+    r = g.run(st, 3, sweep_offset=19910, trace_steps=steps, **kw)
+    n_ex = 0
+    for row in (0, 585, 1170, 2049, 2341, 2926, 3511, 4095):
+        rr = {k: r[k][row:row + 1] for k in ("trace_acc", "trace_prop", "trace_dE")}
+        chk = _follow_check(m, s1[row:row + 1], rr, steps, sweep_offset=19910, **dict(kw, chain_offset=row))
+        assert chk["n_diff"] == 0
+        n_ex += int(chk["exact"].sum())
+        assert 0.0 < chk["acc"].mean() < 0.5
+    print("cfg2 cold end: %d of %d sampled steps decided by the fp64 path" % (n_ex, 8 * steps))
 
 
 def test_error_codes(amh, torch, synth):
