@@ -52,7 +52,8 @@ struct amh_ctx {
     amh_launch_options lopt;
     float2 *Epk = nullptr;       // upper-triangle lerp table (see DevModel)
     float *Elast = nullptr;
-    float *Epl = nullptr;        // the same E, plain rows padded to row_stride floats (TMA source)
+    float *Ebd = nullptr;        // the band j - i <= band_dmax of the same E', column-major, rows padded to row_stride floats (TMA source)
+    int band_dmax = 0;
     float *P = nullptr;          // the probabilities themselves (fp64 path of the exact-decision guard)
     int device = 0, n_sm = 0, max_smem = 0;
     // staging for the *_host calls (grow-only)
@@ -164,6 +165,8 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.c0 = (float)(e0 + 0.5 * delta);
     m.inv_delta = (float)(1.0 / delta);
     m.tmax = (float)(n_bins - 1);
+    m.thmax = (float)n_bins - 1.75f;
+    m.v_far = 0.0;
     m.t0 = (float)(-(e0 + 0.5 * delta) / delta);
     {
         // smallest fp32 d^2 from which pair_energy()'s t is surely clamped to tmax: the last bin centre with a
@@ -192,10 +195,11 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.cbB = m.loc[3][1] / m.loc[2][1];
     m.cbC = m.loc[3][2] / m.loc[2][1];
 
-    if (amh::sweep_smem_bytes(n_res, 1, 0, 0, 0, 0) > (size_t)c->max_smem) {
+    if (n_bins > (1 << 20)) { delete c; return fail(AMH_ERR_UNSUPPORTED, "amh_create: n_bins = %d > 2^20", n_bins); }
+    if (amh::sweep_smem_bytes(n_res, 1, 0, 0, 0, 0, 1, 1) > (size_t)c->max_smem) {
         delete c;
         return fail(AMH_ERR_UNSUPPORTED, "amh_create: L = %d needs %zu B of shared memory per chain, device allows %d",
-                    n_res, amh::sweep_smem_bytes(n_res, 1, 0, 0, 0, 0), c->max_smem);
+                    n_res, amh::sweep_smem_bytes(n_res, 1, 0, 0, 0, 0, 1, 1), c->max_smem);
     }
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -211,7 +215,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
         if (bad_dev) cudaFree(bad_dev);
         if (c->Epk) cudaFree(c->Epk);
         if (c->Elast) cudaFree(c->Elast);
-        if (c->Epl) cudaFree(c->Epl);
+        if (c->Ebd) cudaFree(c->Ebd);
         if (c->P) cudaFree(c->P);
         delete c;
     };
@@ -232,8 +236,14 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
         while ((stride & 7) != 4) stride += 4;          // 16-byte multiple, bank offset 4 (mod 8) words per row
         m.row_stride = stride;
     }
-    AMH_CUDA_C(cudaMalloc(&c->Epl, sizeof(float) * n_rows * m.row_stride));
-    AMH_CUDA_C(cudaMemsetAsync(c->Epl, 0, sizeof(float) * n_rows * m.row_stride, st));
+    // the band of the local phase: pairs up to 64 residues apart (windows up to 32 residues); wider windows gather from L2
+    c->band_dmax = std::min(n_res - 1, 64);
+    m.band_rows = std::max(0, c->band_dmax - o.min_sep + 1);
+    {
+        const size_t bb = sizeof(float) * std::max<size_t>(1, (size_t)n_res * m.band_rows) * m.row_stride;
+        AMH_CUDA_C(cudaMalloc(&c->Ebd, bb));
+        AMH_CUDA_C(cudaMemsetAsync(c->Ebd, 0, bb, st));
+    }
     AMH_CUDA_C(cudaMalloc(&c->P, sizeof(float) * n_rows * n_bins));
     AMH_CUDA_C(cudaMalloc(&bad_dev, sizeof(int)));
     AMH_CUDA_C(cudaMemsetAsync(bad_dev, 0, sizeof(int), st));
@@ -246,8 +256,18 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     {
         const int threads = 256;
         const int blocks = (int)std::min<long long>((count + threads - 1) / threads, (long long)c->n_sm * 16);
-        amh::table_kernel<<<blocks, threads, 0, st>>>(src, c->Epk, c->Elast, c->Epl, c->P, m.row_stride, n_res, n_bins, o.eps, bad_dev);
+        amh::table_kernel<<<blocks, threads, 0, st>>>(src, c->Epk, c->Elast, c->Ebd, m.band_rows, o.min_sep, c->P, m.row_stride, n_res, n_bins, o.eps, bad_dev);
         AMH_CUDA_C(cudaGetLastError());
+    }
+    double *vfar_dev = nullptr;
+    AMH_CUDA_C(cudaMalloc(&vfar_dev, sizeof(double)));
+    amh::vfar_kernel<<<1, 1024, 0, st>>>(c->P, n_res, n_bins, o.min_sep, o.eps, vfar_dev);
+    {
+        cudaError_t e_ = cudaGetLastError();
+        if (e_ == cudaSuccess) e_ = cudaMemcpyAsync(&m.v_far, vfar_dev, sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e_ == cudaSuccess) e_ = cudaStreamSynchronize(st);
+        cudaFree(vfar_dev);
+        if (e_ != cudaSuccess) { cleanup(); return fail(AMH_ERR_CUDA, "amh_create: v_far: %s", cudaGetErrorString(e_)); }
     }
     int bad = 0;
     AMH_CUDA_C(cudaMemcpyAsync(&bad, bad_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -255,7 +275,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     if (bad) { cleanup(); return fail(AMH_ERR_INVALID_ARG, "amh_create: the distogram holds a negative, NaN or infinite value"); }
     cudaFree(bad_dev); bad_dev = nullptr;
     if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
-    m.Epk = c->Epk; m.Elast = c->Elast; m.Epl = c->Epl; m.P = c->P;
+    m.Epk = c->Epk; m.Elast = c->Elast; m.Ebd = c->Ebd; m.P = c->P;
 #define AMH_SMEM_ATTR(SG_, RING_, CB_) AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<SG_, RING_, CB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem))
     AMH_SMEM_ATTR(false, false, false); AMH_SMEM_ATTR(false, false, true); AMH_SMEM_ATTR(false, true, false); AMH_SMEM_ATTR(false, true, true);
     AMH_SMEM_ATTR(true, false, false); AMH_SMEM_ATTR(true, false, true); AMH_SMEM_ATTR(true, true, false); AMH_SMEM_ATTR(true, true, true);
@@ -272,7 +292,7 @@ amh_status amh_destroy(amh_ctx *c)
     // cudaFree waits for the work that still uses the allocation: no device-wide synchronisation of our own
     if (c->Epk) cudaFree(c->Epk);
     if (c->Elast) cudaFree(c->Elast);
-    if (c->Epl) cudaFree(c->Epl);
+    if (c->Ebd) cudaFree(c->Ebd);
     if (c->P) cudaFree(c->P);
     if (c->stage) cudaFree(c->stage);
     delete c;
@@ -322,8 +342,9 @@ amh_status amh_coords(amh_ctx *c, const float *states, long long B, float *cb_ou
     return AMH_OK;
 }
 
-// Launch shape of amh_run: C chains per CTA, W warps per chain, R ring slots.
-struct SweepShape { int C, W, R, ring_rows, cb64; size_t smem; };
+// Launch shape of amh_run: C chains per CTA, W warps per chain, R ring slots, local proposals
+// per pass, lanes per local proposal.
+struct SweepShape { int C, W, R, ring_rows, cb64, nspec, gl, wpts; size_t smem; };
 
 static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
 {
@@ -332,34 +353,54 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
     const int span = std::min(2 * window, std::max(L - 1, 0));
     SweepShape sh;
     sh.ring_rows = std::max(0, span - c->m.min_sep + 1);
+    sh.wpts = w_eff + 1;
+    sh.gl = c->lopt.lanes_per_step > 0 ? c->lopt.lanes_per_step : 8;
     const size_t budget = (size_t)c->max_smem;
-    auto ring_for = [&](int C) -> int {                       // slots: the window's columns + prefetch + drift between teams
-        if (c->lopt.ring_cols < 0 || sh.ring_rows == 0) return 0;
+    auto spec_for = [&](int W) -> int {                       // local proposals per pass the team's lane groups can hold
+        int ns = std::min(W * (32 / sh.gl), amh::kMaxSpec);
+        if (c->lopt.spec_local > 0) ns = std::min(ns, c->lopt.spec_local);
+        ns = std::min(ns, std::max(1, 8192 / (16 * sh.wpts)));    // the turned C-betas of a pass: 8 KB per chain at most
+        return std::max(1, ns);
+    };
+    auto ring_for = [&](int C, int ns) -> int {               // slots: the window's columns + reach of a pass + drift between teams
+        if (c->lopt.ring_cols < 0 || sh.ring_rows == 0 || span > c->band_dmax || c->m.min_sep > amh::kRingPadRows + 1) return 0;
         if (c->lopt.ring_cols > 0) return std::max(c->lopt.ring_cols, w_eff + 3);
-        return w_eff + 3 + amh::kMaxSpec / 2 + (C > 1 ? 4 : 0);    // + reach of a speculative pass + drift between teams
+        return w_eff + 3 + (ns + 1) / 2 + (C > 1 ? 4 : 0);
     };
     sh.cb64 = 1;
-    auto fits = [&](int C, int, int R) { return amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride, sh.cb64) <= budget; };
+    auto fits = [&](int C, int R, int ns) { return amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride, sh.cb64, ns, sh.wpts) <= budget; };
     // chains per CTA: spread the batch over the SMs (one CTA each) and keep as many teams resident as shared memory
     // allows; the ring is added only when it fits beside them (warps in flight are worth more than the ring)
     int C = c->lopt.chains_per_cta;
-    if (C <= 0) {
-        C = (int)std::min<long long>(7, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));    // 7 x 2 warps + producer
+    const bool auto_c = C <= 0;
+    if (auto_c) C = (int)std::min<long long>(7, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));    // 7 x 2 warps + producer
+    auto warps_for = [&](int C_) {
+        const int W = c->lopt.warps_per_chain;
+        return W > 0 ? std::max(1, std::min(W, amh::kMaxTeamWarps / C_)) : std::max(1, std::min(amh::kMaxTeamWarps / C_, 8));
+    };
+    if (auto_c) {
         // the fp64 C-betas (24 L bytes per chain) are dropped before a chain is (they can be rebuilt from N, CA, C)
-        if (!fits(C, 0, 0)) sh.cb64 = 0;
-        while (C > 1 && !fits(C, 0, 0)) --C;
+        if (!fits(C, 0, spec_for(warps_for(C)))) sh.cb64 = 0;
+        while (C > 1 && !fits(C, 0, spec_for(warps_for(C)))) --C;
     }
-    int W = c->lopt.warps_per_chain;
-    W = W > 0 ? std::max(1, std::min(W, amh::kMaxTeamWarps / C)) : std::max(1, std::min(amh::kMaxTeamWarps / C, 8));
-    int R = ring_for(C);
-    if (R > 0 && !fits(C, W, R)) {
-        R = ring_for(1);                                     // without the slack for drift between teams
-        if (!fits(C, W, R)) R = 0;                           // the ring does not fit: rows are gathered from L2
+    const int W = warps_for(C);
+    int ns = spec_for(W);
+    if (sh.cb64 && !fits(C, 0, ns)) sh.cb64 = 0;             // forced shapes
+    int R = ring_for(C, ns);
+    if (R > 0 && !fits(C, R, ns)) {
+        if (sh.cb64) { sh.cb64 = 0; }                        // the ring is worth more than the stored fp64 C-betas
+        if (!fits(C, R, ns)) {
+            R = ring_for(1, ns);                             // without the slack for drift between teams
+            if (!fits(C, R, ns)) { R = 0; sh.cb64 = fits(C, 0, ns) ? sh.cb64 : 0; }   // the ring does not fit: rows are gathered from L2
+        }
     }
-    sh.C = C; sh.W = W; sh.R = R;
+    if (R == 0 && !sh.cb64) { sh.cb64 = 1; if (!fits(C, 0, ns)) sh.cb64 = 0; }
+    // a pass may not reach beyond what the ring can hold next to the window (else the team would wait for a column
+    // whose slot it still occupies itself)
+    if (R > 0) ns = std::max(1, std::min(ns, 2 * (R - w_eff - 2) - 1));
+    sh.C = C; sh.W = W; sh.R = R; sh.nspec = ns;
     if (R == 0) sh.ring_rows = 0;
-    if (sh.cb64 && !fits(C, W, 0)) sh.cb64 = 0;              // forced shapes
-    sh.smem = amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride, sh.cb64);
+    sh.smem = amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride, sh.cb64, ns, sh.wpts);
     return sh;
 }
 
@@ -451,8 +492,7 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
         return fail(AMH_ERR_UNSUPPORTED, "amh_run: L = %d, window = %d, %d chains x %d warps need %zu B of shared memory, device allows %d",
                     c->m.L, sc->window, sh.C, sh.W, sh.smem, c->max_smem);
     a.C = sh.C; a.W = sh.W; a.ring_cols = sh.R; a.ring_rows = sh.ring_rows; a.cb64 = sh.cb64;
-    a.spec_local = c->lopt.spec_local;
-    a.lanes_per_step = c->lopt.lanes_per_step > 0 ? c->lopt.lanes_per_step : 8;
+    a.nspec = sh.nspec; a.lanes_per_step = sh.gl; a.wpts = sh.wpts;
     const long long ctas = (B + sh.C - 1) / sh.C;
     // global proposals: one warp per step, speculatively, when a team has few warps (the whole team on one step when it
     // has many: a speculative pass of W steps wastes the ones after the first accept)

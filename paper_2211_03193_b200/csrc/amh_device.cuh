@@ -22,21 +22,29 @@ struct Xf {            // x -> R x + t, R row-major
 
 struct DevModel {
     int L, nb, min_sep, n;           // residues, bins, minimum sequence separation, variables (2L)
-    // Energy table, upper triangle only (R9: only p[i][j], i < j, is read).  Row r = tri(i, j) of pair i < j:
-    //   Epk[r][b]   = { E[b], E[min(b+1, nb-1)] - E[b] },  E = -log(p + eps)   (the two operands of R8's lerp)
-    //   Elast[r]    = e_ij(d) for every d >= the last bin centre (the clamped value of R8)
-    //   Epl[r][b]   = E[b], rows padded to row_stride floats (16-byte multiples whose bank offset differs from row
-    //                 to row): what the TMA bulk copies stage into shared memory for the local phase
+    // Energy table, upper triangle only (R9: only p[i][j], i < j, is read).  Row r = tri(i, j) of pair i < j.
+    // With E = -log(p + eps) and Elast = E[nb-1] (the value R8's clamp gives to every d >= the last bin centre), the
+    // tables hold the EXCESS E'[b] = fp32(E[b] - Elast) (E'[nb-1] = 0: a far pair's term is exactly 0):
+    //   Epk[r][b]   = { E'[b], E'[min(b+1, nb-1)] - E'[b] }   (the two operands of R8's lerp)
+    //   Elast[r]    = fp32(Elast)
+    //   Ebd[j][q][b] = E'[b] of the pair (j - min_sep - q, j), q = 0 .. band_rows - 1 (the band j - i <= band_dmax), rows
+    //                 padded to row_stride floats (16-byte multiples whose bank offset differs from row to row), zero
+    //                 where i < 0: a COLUMN of the local phase is one contiguous block, staged into shared memory by one
+    //                 TMA bulk copy
+    //   v_far       = sum over the pairs j - i >= min_sep of Elast (fp64): V = v_far + sum of the excess terms
     //   P[r][b]     = p_ij(b) as given (fp32): the fp64 path of the exact-decision guard takes -log(p + eps) itself
     const float2 *Epk;
     const float *Elast;
-    const float *Epl;
+    const float *Ebd;
+    int band_rows;                   // rows per column of Ebd: band_dmax - min_sep + 1 (0 = no band)
     const float *P;
     int row_stride;
     double c0_d, delta_d, eps_d;     // first bin centre, bin width, eps in fp64 (fp64 path)
     double far2_d;                   // squared distance from which the fp64 path is surely clamped (last centre + margin)
     float c0, inv_delta, tmax;       // first bin centre, 1/bin width, nb-1
     float t0;                        // -c0 / bin width
+    float thmax;                     // nb - 1.75 (bin_frac)
+    double v_far;
     float dfar;                      // >= sqrt(far2)
     float far2;                      // d^2 >= far2  =>  the clamp of R8 applies: e_ij(d) = Elast
     // bond-frame recursion H_{i+1} = H_i * A * Mplus(theta2, psi_i) * W * Rx(phi_{i+1})
@@ -196,8 +204,8 @@ __device__ __forceinline__ void nerf_build_warp(const DevModel &m, const float *
 }
 
 // ------------------------------------------------------------------------------------------------
-// Pair term (Eq. 3a, R8): linear interpolation of E between bin centres, clamped at the end centres.
-// d2 = 0 is safe (IEEE sqrt), so coincident atoms score E[0].
+// Excess pair term e'(d) = e(d) - Elast (Eq. 3a, R8): linear interpolation between bin centres, clamped at the end
+// centres.  d2 = 0 is safe (IEEE sqrt), so coincident atoms score E'[0].
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float pair_energy(const float2 *__restrict__ row, float d2, float c0, float inv_delta, float tmax, int nb)
 {

@@ -10,7 +10,8 @@ namespace amh {
 // a0  E = -log(p + eps)   (Eq. 3a; BASELINE.json:7's 1e-8)
 // ------------------------------------------------------------------------------------------------
 __global__ void table_kernel(const float *__restrict__ p, float2 *__restrict__ Epk, float *__restrict__ Elast,
-                             float *__restrict__ Epl, float *__restrict__ P, int row_stride, int L, int nb, double eps, int *__restrict__ bad)
+                             float *__restrict__ Ebd, int band_rows, int min_sep, float *__restrict__ P, int row_stride, int L, int nb, double eps,
+                             int *__restrict__ bad)
 {
     const long long count = (long long)L * L * nb;
     const long long stride = (long long)gridDim.x * blockDim.x;
@@ -22,16 +23,38 @@ __global__ void table_kernel(const float *__restrict__ p, float2 *__restrict__ E
         const long long ij = q / nb;
         const int i = (int)(ij / L), j = (int)(ij % L);
         if (j <= i) continue;                                        // R9: only i < j is read
-        const float e0 = (float)(-log((double)v + eps));
-        const float e1 = (b + 1 < nb) ? (float)(-log((double)p[q + 1] + eps)) : e0;
+        // excess over the clamped value of the row (DevModel): E'[nb-1] = 0 exactly
+        const double elast = -log((double)p[q - b + nb - 1] + eps);
+        const float e0 = (float)(-log((double)v + eps) - elast);
+        const float e1 = (b + 1 < nb) ? (float)(-log((double)p[q + 1] + eps) - elast) : e0;
         const float de = e1 - e0;
         const long long r = tri_base(i, L) + j;
         Epk[r * nb + b] = make_float2(e0, de);
-        Epl[r * row_stride + b] = e0;
+        const int q_ = j - i - min_sep;
+        if (q_ >= 0 && q_ < band_rows) Ebd[((long long)j * band_rows + q_) * row_stride + b] = e0;
         P[r * nb + b] = v;
-        if (b == nb - 2) Elast[r] = fmaf(1.0f, de, e0);              // the value pair_energy() returns at t = tmax
+        if (b == nb - 1) Elast[r] = (float)elast;
     }
     if (local_bad) atomicOr(bad, 1);
+}
+
+// v_far = sum over the pairs j - i >= min_sep of -log(p[nb-1] + eps) in fp64 (one block, fixed order: deterministic)
+__global__ void __launch_bounds__(1024) vfar_kernel(const float *__restrict__ P, int L, int nb, int min_sep, double eps, double *__restrict__ out)
+{
+    __shared__ double sh[1024];
+    double acc = 0.0;
+    for (int i = 0; i < L; ++i) {
+        const long long rb = tri_base(i, L);
+        for (int j = i + min_sep + (int)threadIdx.x; j < L; j += (int)blockDim.x)
+            acc += -log((double)P[(rb + j) * nb + nb - 1] + eps);
+    }
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int d = 512; d > 0; d >>= 1) {
+        if ((int)threadIdx.x < d) sh[threadIdx.x] += sh[threadIdx.x + d];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sh[0];
 }
 
 __global__ void philox_test_kernel(const uint32_t *ctr, const uint32_t *key, uint32_t *out, long long count)
@@ -66,7 +89,7 @@ __global__ void __launch_bounds__(128) coords_kernel(DevModel m, const float *__
 // shared: float cb[3][L], double red[32]
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double energy_range_cta(const DevModel &m, const float *cbx, const float *cby,
-                                                   const float *cbz, int lo, int hi, int warp, int nwarps, int lane)
+                                                   const float *cbz, int lo, int hi, bool whole, int warp, int nwarps, int lane)
 {
     double e = 0.0;
     for (int i = lo + warp; i <= hi; i += nwarps) {
@@ -75,9 +98,10 @@ __device__ __forceinline__ double energy_range_cta(const DevModel &m, const floa
         for (int j = i + m.min_sep + lane; j <= hi; j += 32) {
             const float dx = xi - cbx[j], dy = yi - cby[j], dz = zi - cbz[j];
             const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-            // far pairs take the clamped value from the compact array (coalesced in j), near pairs gather their row
-            e += (double)((d2 >= m.far2) ? __ldg(m.Elast + rb + j)
-                                         : pair_energy(m.Epk + (rb + j) * m.nb, d2, m.c0, m.inv_delta, m.tmax, m.nb));
+            // a window's pairs take their clamped value from the compact array (coalesced in j; the whole chain's are
+            // v_far), near pairs add their excess
+            if (!whole) e += (double)__ldg(m.Elast + rb + j);
+            if (d2 < m.far2) e += (double)pair_energy(m.Epk + (rb + j) * m.nb, d2, m.c0, m.inv_delta, m.tmax, m.nb);
         }
     }
     return e;
@@ -100,13 +124,13 @@ __global__ void __launch_bounds__(128) energy_kernel(DevModel m, const float *__
         __syncthreads();
         int lo = 0, hi = m.L - 1;
         if (k >= 0) { const int c = k >> 1; lo = max(0, c - window); hi = min(m.L - 1, c + window); }
-        double e = warp_sum(energy_range_cta(m, cbx, cby, cbz, lo, hi, warp, nwarps, lane));
+        double e = warp_sum(energy_range_cta(m, cbx, cby, cbz, lo, hi, k < 0, warp, nwarps, lane));
         if (lane == 0) red[warp] = e;
         __syncthreads();
         if (threadIdx.x == 0) {
             double tot = 0.0;
             for (int w = 0; w < nwarps; ++w) tot += red[w];
-            out[row] = (float)tot;
+            out[row] = (float)(k < 0 ? m.v_far + tot : tot);
         }
         __syncthreads();
     }

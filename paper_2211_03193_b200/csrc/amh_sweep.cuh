@@ -4,25 +4,37 @@
 // barrier; one more warp (the last) is the PRODUCER that feeds the table ring by TMA bulk copies.
 // Chains are independent: teams never wait for one another except through the ring.
 //
-// Global sweeps (Eq. 1, 3a): O(L^2/6) straddling pairs per proposal, evaluated either by the whole team one
-// proposal at a time (SG = false) or speculatively like the local ones, one warp per step (SG = true).  A thread owns a column j: it turns CB_j itself and walks the rows i in blocks of 8; a block
-// whose bounding sphere is beyond the last bin centre for both positions of CB_j is skipped whole, pairs
-// clamped before and after are skipped one by one (their term is exactly 0), near pairs gather 8 bytes
-// from the packed table in L2, four rows' gathers in flight at a time.
+// What a proposal costs.  dE = S_new - S_old, both sums over the pairs that straddle the
+// flipped bond (all of them in a global sweep, Eq. 1/3a; the in-window ones in a local sweep, Eq. 2/3b), of the
+// EXCESS pair energy e'_ij(d) = e_ij(d) - e_ij(infinity) (0 beyond the last bin centre, so far pairs drop out of
+// both sums exactly).  Only S_new is evaluated pair by pair.  S_old is carried from step to step: when the step
+// index advances, the set of straddling pairs changes by one row and one column (O(w) or O(L) pairs, the
+// "transition" T(k)); when a proposal is accepted, S_old becomes that proposal's S_new.
 //
-// Local sweeps (Eq. 2, 3b): a proposal has only ~65-150 pairs, and Alg. 1 orders the proposals of a
-// chain strictly.
+// Local sweeps: a proposal has only ~70-150 pairs and Alg. 1 orders the proposals of a chain strictly
+// (PAPER.md:105, 114).
 //   * Speculation.  The draws are counter-based (R6), so the proposals of steps k, k+1, ... are known in
 //     advance: GROUP r (8, 16 or 32 lanes; up to 16 groups per team) evaluates step k+r AGAINST THE
 //     CURRENT STATE, and the results are consumed in order up to and including the first accepted step;
 //     later results were computed against a state that no longer exists and are thrown away (their steps
 //     are evaluated again in the next pass).  The trajectory is exactly the sequential one.
+//   * A group first turns the <= w+1 C-betas right of its bond (fp64, rounded once) into shared memory, then
+//     deals the nI x nJ pairs of the step evenly to its lanes (pair p = lane, lane + gl, ...).
 //   * Table ring.  Every chain of the CTA walks k = 0..n-1, so they all need the same table rows at about
 //     the same time: pair (i, j) is needed while the window centre c is in [max(i, j-w), min(j, i+w)].
 //     The producer streams "column" j = the rows (i, j), j-2w <= i <= j-min_sep, into slot q mod R of a
 //     shared-memory ring (q = a running column number) with cp.async.bulk + mbarrier complete_tx; teams
-//     wait on the slot's barrier, gather from shared memory (32 banks instead of one L1 wavefront per
-//     lane) and publish their progress; a slot is refilled once every team has passed its column.
+//     wait on the slot's "full" barrier, read from shared memory, and arrive on the slot's "empty" barrier
+//     once the column is dead for them; the producer refills a slot when every team has arrived.
+//
+// Global sweeps: O(L^2/6) straddling pairs per proposal, evaluated either by the whole team one proposal at a
+// time (SG = false) or speculatively, one warp per step (SG = true).  A thread owns a column j: it turns CB_j
+// itself and walks the rows i in blocks of 8; a block whose bounding sphere is beyond the last bin centre of
+// the new CB_j is skipped whole, far pairs are skipped one by one, near pairs gather 8 bytes from the packed
+// table in L2, four rows' gathers in flight at a time.
+//
+// Exact-decision guard (R24): the sums are fp32; a proposal whose gap |log u + dE/T| is inside the bound on
+// their error is evaluated again in fp64 from the fp64 atoms and the probabilities themselves before deciding.
 #pragma once
 #include "amh_device.cuh"
 
@@ -40,10 +52,11 @@ struct RunArgs {
     long long ramp_sigma;
     // launch shape
     int C, W;                            // chains per CTA, warps per chain
-    int spec_local;                      // local proposals evaluated per pass (<= W * 32 / lanes_per_step, <= 16)
+    int nspec;                           // local proposals evaluated per pass (<= W * 32 / lanes_per_step, <= 16)
     int lanes_per_step;                  // lanes that share one local proposal: 32, 16 or 8
     int ring_cols;                       // R: slots of the table ring (> window + 2), 0 = gather from L2 instead
     int ring_rows;                       // rows per column: 2w - min_sep + 1
+    int wpts;                            // C-betas a local proposal turns, at most: min(window, L-1) + 1
     int cb64;                            // fp64 C-betas kept in shared memory (else rebuilt from N, CA, C)
     unsigned long long seed;
     double guard_local, guard_global;    // exact-decision guard: bound on the fp32 error of dE at 32 A extent (0 = off)
@@ -59,36 +72,45 @@ struct RunArgs {
 
 constexpr int kDrawBatch = 64;           // steps whose draws are generated together, two per lane
 constexpr int kMaxWarps = 16;            // array bound of the per-warp scratch of a team
-constexpr int kMaxSpec = 16;             // local proposals evaluated per pass, at most
+constexpr int kMaxSpec = 16;             // proposals evaluated per pass, at most
 constexpr int kBlk = 8;                  // residues per culling block of the global phase
 constexpr int kMaxTeamWarps = 15;        // team warps per CTA: chains x warps per chain (+ the producer = 512 threads)
 constexpr int kMaxChains = 15;           // chains per CTA (named barriers 1..15)
 constexpr int kSweepMaxThreads = 512;    // 15 team warps + the producer: 128 registers per thread
+constexpr int kRingPadRows = 4;          // rows in front of the first ring slot that masked-off evaluations (j - i < min_sep) may touch
 
 // shared memory of one chain, in bytes (a multiple of 16):
 //   double X[aL], Y[aL], Z[aL]   atoms, index atom * L + res (atom 0..2 = N, CA, C; a = 3).  The C-beta is a fixed
 //                                combination of the three (cb_point); it is kept in fp64 too (atom 3, a = 4) when
 //                                that does not cost a resident chain (cb64), else rebuilt where needed
-//   double red[16], b_cd[64], b_sd[64], b_lu[64], rot_s[16][12], sp_dE[16]
-//   float4 cb4[L]                fp32 copy of the C-betas (what the pair loops read)
+//   double red[32], b_cd[64], b_sd[64], b_lu[64], rot_s[16][12], sp_new[16], sp_T[16]
+//   float4 cb4[L]                fp32 copy of the C-betas (what the pair loops read); .w = byte offset of the
+//                                residue's term in a table address (as the ROW index i of a pair)
 //   float4 blk4[ceil(L/8)]       bounding spheres of 8-residue blocks (culling in the global phase)
-//   float  s[n], b_sp[64];  int sp_acc[16]
-__host__ __device__ inline size_t chain_smem_bytes(int L, int cb64)
+//   float4 cbn[nspec][wpts]      the turned C-betas of the local proposals of a pass; .w = the column's term
+//   float  s[n], b_sp[64]
+__host__ __device__ inline size_t chain_smem_bytes(int L, int cb64, int nspec, int wpts)
 {
-    const size_t doubles = (cb64 ? 12 : 9) * (size_t)L + (cb64 ? 0 : (L & 1)) + kMaxWarps + 3 * kDrawBatch + 12 * kMaxSpec + kMaxSpec;   // (L & 1): cb4 on 16 bytes
-    size_t floats = 4 * (size_t)L + 4 * (((size_t)L + kBlk - 1) / kBlk) + 2 * (size_t)L + kDrawBatch + kMaxSpec;
+    size_t doubles = (cb64 ? 12 : 9) * (size_t)L;
+    doubles += doubles & 1;                                  // float4 arrays on 16 bytes
+    doubles += 2 * kMaxWarps + 3 * kDrawBatch + 12 * kMaxSpec + 2 * kMaxSpec;
+    size_t floats = 4 * (size_t)L + 4 * (((size_t)L + kBlk - 1) / kBlk) + 4 * (size_t)nspec * wpts + 2 * (size_t)L + kDrawBatch;
     floats = (floats + 3) & ~(size_t)3;
     return sizeof(double) * doubles + sizeof(float) * floats;
 }
 
-// header: ring barriers, progress words; then the ring; then the chains
-__host__ __device__ inline size_t sweep_header_bytes(int ring_cols) { return (8 * (size_t)ring_cols + 8 * 16 + 15) & ~(size_t)15; }
+// header: full barriers [R], empty barriers [R]; then the ring; then the chains
+__host__ __device__ inline size_t sweep_header_bytes(int ring_cols) { return (16 * (size_t)ring_cols + 15) & ~(size_t)15; }
 
-__host__ __device__ inline size_t sweep_smem_bytes(int L, int C, int ring_cols, int ring_rows, int row_stride, int cb64)
+__host__ __device__ inline size_t ring_bytes(int ring_cols, int ring_rows, int row_stride)
 {
-    size_t b = sweep_header_bytes(ring_cols) + sizeof(float) * (size_t)ring_cols * ring_rows * row_stride;
-    b = (b + 15) & ~(size_t)15;
-    return b + (size_t)C * chain_smem_bytes(L, cb64);
+    if (ring_cols <= 0) return 0;
+    return (sizeof(float) * ((size_t)ring_cols * ring_rows + kRingPadRows) * row_stride + 15) & ~(size_t)15;
+}
+
+__host__ __device__ inline size_t sweep_smem_bytes(int L, int C, int ring_cols, int ring_rows, int row_stride, int cb64, int nspec, int wpts)
+{
+    return sweep_header_bytes(ring_cols) + ring_bytes(ring_cols, ring_rows, row_stride) + (size_t)C * chain_smem_bytes(L, cb64, nspec, wpts);
 }
 
 // ---- PTX: mbarrier, TMA bulk copy, named barriers ----------------------------------------------------
@@ -102,9 +124,10 @@ __device__ __forceinline__ void mbar_expect_tx(void *bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+// arrive (release at CTA scope: the caller's earlier reads of the slot are ordered before it)
 __device__ __forceinline__ void mbar_arrive(void *bar)
 {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+    asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
 {
@@ -112,7 +135,7 @@ __device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
     uint32_t ok;
     do {
         // the last operand lets the hardware park the thread for up to ~1 us instead of spinning on the barrier
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(ok) : "r"(a), "r"(parity), "r"(1000u) : "memory");
     } while (!ok);
 }
@@ -169,27 +192,23 @@ __device__ __forceinline__ void cb_point(const DevModel &m, const double *X, con
     z = fma(m.cbC, fma(ex, vy, -ey * vx), fma(m.cbB, vz, fma(m.cbA, ez, az)));
 }
 
-// bin index and fraction of R8's interpolation at squared distance d2.  d = sqrt.approx.f32(d2): one MUFU instruction,
-// maximum relative error 2^-23 (PTX ISA), i.e. within 1 ulp of the correctly rounded root (the
-// coordinates feeding d2 are themselves rounded to fp32), instead of sqrtf()'s 9 instructions with its special-case
-// branch; d2 = 0 (coincident atoms) gives 0 and lands in the first bin.  Rows in the ring are plain E[0..nb-1]: the
-// caller forms E[b+1] - E[b] itself, the same fp32 subtraction the packed table did at create.
-__device__ __forceinline__ void lerp_coords(float d2, float t0, float inv_delta, float tmax, int nb, int &b, float &f)
+// bin index b and fraction f of R8's interpolation at squared distance d2: t = (d - c0) / delta clamped to
+// [0, nb-1], b <= t <= b + 1, b <= nb - 2, f = t - b.
+//   d = sqrt.approx.f32(d2): one MUFU instruction, maximum relative error 2^-23 (PTX ISA); d2 = 0 gives 0.
+//   b = round-to-nearest-even(t - 1/2), read off the low mantissa bits of (t - 1/2) + 1.5 * 2^23: conversion
+//   instructions (F2I, I2F) run at the MUFU rate on sm_100 (16 per clock and SM, measured), these are plain FADDs.
+//   At an integer t either neighbour bin gives the same value (the interpolant is continuous), and
+//   min(t - 1/2, nb - 1.75) keeps b <= nb - 2.
+__device__ __forceinline__ void bin_frac(float d2, float t0, float inv_delta, float tmax, float thmax, int &b, float &f)
 {
     float d;
     asm("sqrt.approx.f32 %0, %1;" : "=f"(d) : "f"(d2));
     float t = fmaf(d, inv_delta, t0);                        // (d - c0) / delta with t0 = -c0 / delta: one fma
     t = fminf(fmaxf(t, 0.0f), tmax);
-    b = min((int)t, nb - 2);
-    f = t - (float)b;
+    const float u = __fadd_rn(fminf(__fadd_rn(t, -0.5f), thmax), 12582912.0f);
+    f = __fadd_rn(t, -__fadd_rn(u, -12582912.0f));
+    b = __float_as_int(u) & 0x3fffff;
 }
-
-// Where the rows of a local proposal come from: the shared-memory ring or, when the ring is off, the
-// packed table in L2.  slot0 = ring slot of column j = split of the step being evaluated.
-struct RowSource {
-    const float *ring;       // nullptr = gather from m.Epk
-    int ring_cols, ring_rows, span, slot0;
-};
 
 // floor(a / b) for 0 <= a < 2^16, 1 <= b < 2^10 without the integer-division sequence
 __device__ __forceinline__ int small_div(int a, int b)
@@ -200,18 +219,149 @@ __device__ __forceinline__ int small_div(int a, int b)
 // row index of the pair i < j in 32 bits (L < 46341)
 __device__ __forceinline__ int tri_row(int i, int j, int L) { return (i * (2 * L - i - 1)) / 2 - i - 1 + j; }
 
-// sum over the pairs (i, j), ilo <= i < split <= j <= jhi, j - i >= min_sep, of e(new) - e(old), where new = the
-// C-beta of j turned by R.  Work is dealt to `nthr` threads, this one being `tid`: a thread OWNS a column j -
-// it turns CB_j itself (fp64, rounded once to fp32) and keeps both positions in registers - and walks the rows
-// i; when a round has fewer columns than threads, S threads share a column and take every S-th row.
-template <bool RING, bool CULL>
-__device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSource &rs, const float4 *cb4, const float4 *blk4,
-                                                 const double *X, const double *Y, const double *Z, bool cb64, const Rot &R,
-                                                 int ilo, int split, int jhi, int tid, int nthr)
+// ---- local phase: tables addressed as base + rowterm(i) + colterm(j) + bin ----------------------------------
+// RING: rows of plain E' in the shared-memory ring, row j - i - min_sep of slot(j): rowterm = -i * row_stride * 4,
+// colterm = ((slot(j) * ring_rows + j - min_sep) * row_stride) * 4.
+// else: packed {E', dE'} in L2: rowterm = tri_base(i) * nb * 8, colterm = j * nb * 8.
+struct LocalTab {
+    const unsigned char *base;
+    int ring_cols, ring_rows, min_sep, stride4;              // stride4 = row_stride * 4 (RING)
+    int slot_c, c_ref;                                       // ring slot of column c_ref (RING)
+    int nb8;                                                 // nb * 8 (L2)
+};
+
+template <bool RING>
+__device__ __forceinline__ int col_term(const LocalTab &tb, int j)
 {
-    const int nJ = jhi - split + 1;
+    if (RING) {
+        int s = tb.slot_c + (j - tb.c_ref);                  // 0 <= j - c_ref < ring_cols: one wrap at most
+        if (s >= tb.ring_cols) s -= tb.ring_cols;
+        return (s * tb.ring_rows + j - tb.min_sep) * tb.stride4;
+    }
+    return j * tb.nb8;
+}
+
+// excess energy e'_ij of one pair from its two points; ci.w / pj.w carry the row / column terms of the address
+template <bool RING>
+__device__ __forceinline__ float local_pair(const DevModel &m, const LocalTab &tb, const float4 ci, const float4 pj)
+{
+    const float dx = ci.x - pj.x, dy = ci.y - pj.y, dz = ci.z - pj.z;
+    const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+    int b;
+    float f;
+    bin_frac(d2, m.t0, m.inv_delta, m.tmax, m.thmax, b, f);
+    const unsigned char *row = tb.base + (__float_as_int(ci.w) + __float_as_int(pj.w));
+    if (RING) {
+        const float *r = reinterpret_cast<const float *>(row) + b;
+        const float e0 = r[0], e1 = r[1];
+        return fmaf(f, e1 - e0, e0);
+    } else {
+        const float2 v = __ldg(reinterpret_cast<const float2 *>(row) + b);
+        return fmaf(f, v.y, v.x);
+    }
+}
+
+// S_new of a local proposal: sum of e' over the pairs (i, j), ilo <= i < split <= j <= jhi, j - i >= min_sep, with the
+// turned C-betas cbn[j - split].  The nI x nJ pairs are dealt to the gl lanes of the group: pair p = glane + t * gl,
+// i = ilo + p / nJ, j = split + p % nJ.  Returns this lane's partial sum.
+template <bool RING>
+__device__ __forceinline__ float local_new_sum(const DevModel &m, const LocalTab &tb, const float4 *cb4, const float4 *cbn,
+                                               int ilo, int split, int nI, int nJ, int glane, int gl)
+{
+    constexpr int U = 3;
+    const int nP = nI * nJ;
+    float acc[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) acc[u] = 0.0f;
+    if (nP <= 0) return 0.0f;
+    int ii = small_div(glane, nJ), jj = glane - ii * nJ;
+    for (int p = glane; p < nP; p += U * gl) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const bool in = p + u * gl < nP;
+            const int iu = in ? ii : 0, ju = in ? jj : 0;
+            const float4 ci = cb4[ilo + iu];
+            const float4 pj = cbn[ju];
+            const bool valid = in && (split + ju) - (ilo + iu) >= m.min_sep;
+            const float e = local_pair<RING>(m, tb, ci, pj);
+            acc[u] += valid ? e : 0.0f;
+            jj += gl;
+            while (jj >= nJ) { jj -= nJ; ++ii; }
+        }
+    }
+    float s = acc[0];
+#pragma unroll
+    for (int u = 1; u < U; ++u) s += acc[u];
+    return s;
+}
+
+// T(k) = S_old(k) - S_old(k - 1) for the CURRENT state: the straddling set of step k minus that of step k - 1
+// (DESIGN.md section 7 "Transitions").  w >= L - 1 makes the window the whole chain (global sweeps).
+//   k odd  (c = k >> 1): the split moves from c to c + 1: column c leaves (rows lo..c - ms), row c enters (columns c + ms..hi)
+//   k even (c >= 1):     the window moves from c - 1 to c: row c - 1 - w leaves (columns c..c - 1 + w), column c + w enters
+// Each is a line of pairs (i0 + t * di, j0 + t * dj), t < count.
+struct Line { int i0, j0, di, dj, cnt; };
+
+__device__ __forceinline__ void transition_lines(int k, int L, int w, int ms, Line &leave, Line &enter)
+{
+    const int c = k >> 1;
+    leave.cnt = 0; leave.i0 = leave.j0 = leave.di = leave.dj = 0;
+    enter = leave;
+    if (k <= 0) return;
+    if (k & 1) {
+        const int lo = max(0, c - w), hi = min(L - 1, c + w);
+        leave.i0 = lo; leave.j0 = c; leave.di = 1; leave.dj = 0; leave.cnt = max(0, c - ms - lo + 1);
+        enter.i0 = c; enter.j0 = c + ms; enter.di = 0; enter.dj = 1; enter.cnt = max(0, hi - c - ms + 1);
+    } else {
+        const int il = c - 1 - w;
+        if (il >= 0) {
+            const int j0 = max(c, il + ms), j1 = min(L - 1, c - 1 + w);
+            leave.i0 = il; leave.j0 = j0; leave.di = 0; leave.dj = 1; leave.cnt = max(0, j1 - j0 + 1);
+        }
+        const int je = c + w;
+        if (je <= L - 1) {
+            const int i0 = max(0, c - w), i1 = min(c - 1, je - ms);
+            enter.i0 = i0; enter.j0 = je; enter.di = 1; enter.dj = 0; enter.cnt = max(0, i1 - i0 + 1);
+        }
+    }
+}
+
+template <bool RING>
+__device__ __forceinline__ float local_transition(const DevModel &m, const LocalTab &tb, const float4 *cb4, int k, int w,
+                                                  int glane, int gl)
+{
+    Line lv, en;
+    transition_lines(k, m.L, w, m.min_sep, lv, en);
+    float acc = 0.0f;
+    const int tot = lv.cnt + en.cnt;
+    for (int q = glane; q < tot; q += gl) {
+        const bool isl = q < lv.cnt;
+        const int t = isl ? q : q - lv.cnt;
+        const int i = isl ? lv.i0 + t * lv.di : en.i0 + t * en.di;
+        const int j = isl ? lv.j0 + t * lv.dj : en.j0 + t * en.dj;
+        const float4 ci = cb4[i];
+        float4 cj = cb4[j];
+        cj.w = __int_as_float(col_term<RING>(tb, j));
+        const float e = local_pair<RING>(m, tb, ci, cj);
+        acc += isl ? -e : e;
+    }
+    return acc;
+}
+
+// ---- global phase -------------------------------------------------------------------------------------------
+// Sum of e' over the pairs (i, j), i < split, jlo <= j <= jhi, j - i >= min_sep, with CB_j turned by R (turn = true) or
+// left where it is (turn = false: a transition line).  Work is dealt to `nthr` threads, this one being `tid`:
+// a thread OWNS a column j - it turns CB_j itself (fp64, rounded once to fp32) - and walks the rows i in blocks of kBlk
+// residues whose bounding spheres are kept in blk4: a block beyond the last bin centre holds only pairs whose term is
+// exactly 0 and is skipped whole.  When a round has fewer columns than threads, S threads share a column and take
+// every S-th block.
+__device__ __forceinline__ double global_cols_sum(const DevModel &m, const float4 *cb4, const float4 *blk4,
+                                                  const double *X, const double *Y, const double *Z, bool cb64, bool turn, const Rot &R,
+                                                  int split, int jlo, int jhi, int tid, int nthr)
+{
+    const int nJ = jhi - jlo + 1;
     double acc = 0.0;
-    if (split <= ilo || nJ <= 0) return acc;
+    if (split <= 0 || nJ <= 0) return acc;
     for (int c0 = 0; c0 < nJ; c0 += nthr) {
         const int nc = min(nthr, nJ - c0);
         int S = 1, col = tid, slice = 0;
@@ -219,96 +369,81 @@ __device__ __forceinline__ double cross_pairs_dE(const DevModel &m, const RowSou
             S = small_div(nthr, nc); slice = small_div(tid, nc); col = tid - slice * nc;
             if (slice >= S) break;
         }
-        const int j = split + c0 + col;
-        double x0, y0, z0, x, y, z;
-        if (cb64) { x0 = X[3 * m.L + j]; y0 = Y[3 * m.L + j]; z0 = Z[3 * m.L + j]; }
-        else cb_point(m, X, Y, Z, m.L, j, x0, y0, z0);
-        rot_apply(R, x0, y0, z0, x, y, z);
-        const float xn = (float)x, yn = (float)y, zn = (float)z;
-        const float4 o = cb4[j];
-        const int i_end = min(split - 1, j - m.min_sep);
-        const float *colp = nullptr;
-        if (RING) {
-            int slot = rs.slot0 + (j - split);               // nJ <= w + 1 < ring_cols: one wrap at most
-            if (slot >= rs.ring_cols) slot -= rs.ring_cols;
-            colp = rs.ring + ((size_t)slot * rs.ring_rows + (rs.span - j)) * m.row_stride;   // + i * row_stride
-        }
-        // U rows per trip: all distances first, then all gathers, then the sums, so that a thread has 2U loads in
-        // flight instead of stalling on each pair's row (the rows of near pairs come from L2, ~600 cycles away)
-        constexpr int U = 4;
-        auto trip = [&](int i, int stride) {
-            float d2n[U], d2o[U];
-            int iu[U];
-            bool near[U];
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                const int ii = i + u * stride;
-                const bool valid = ii <= i_end;
-                iu[u] = valid ? ii : i;
-                const float4 ci = cb4[iu[u]];
-                float dx = ci.x - xn, dy = ci.y - yn, dz = ci.z - zn;
-                d2n[u] = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                dx = ci.x - o.x; dy = ci.y - o.y; dz = ci.z - o.z;
-                d2o[u] = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                // a pair beyond the last bin centre before and after scores the same clamped value twice:
-                // its term is exactly 0 and its row is never touched
-                // (in the window of a local proposal nearly every pair is near: the test is skipped there and a far
-                // pair goes through the clamped interpolation, which gives the same two values and the same 0)
-                near[u] = valid && (!CULL || d2n[u] < m.far2 || d2o[u] < m.far2);
-            }
-            float fn[U], fo[U];
-            int bn[U], bo[U];
-            if (RING) {
-                float en0[U], en1[U], eo0[U], eo1[U];
-#pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    en0[u] = en1[u] = eo0[u] = eo1[u] = 0.0f;
-                    if (near[u]) {
-                        lerp_coords(d2n[u], m.t0, m.inv_delta, m.tmax, m.nb, bn[u], fn[u]);
-                        lerp_coords(d2o[u], m.t0, m.inv_delta, m.tmax, m.nb, bo[u], fo[u]);
-                        const float *rowp = colp + iu[u] * m.row_stride;
-                        en0[u] = rowp[bn[u]]; en1[u] = rowp[bn[u] + 1];
-                        eo0[u] = rowp[bo[u]]; eo1[u] = rowp[bo[u] + 1];
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < U; ++u)
-                    if (near[u]) acc += (double)(fmaf(fn[u], en1[u] - en0[u], en0[u]) - fmaf(fo[u], eo1[u] - eo0[u], eo0[u]));
-            } else {
-                float2 vn[U], vo[U];
-#pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    vn[u] = vo[u] = make_float2(0.0f, 0.0f);
-                    if (near[u]) {
-                        lerp_coords(d2n[u], m.t0, m.inv_delta, m.tmax, m.nb, bn[u], fn[u]);
-                        lerp_coords(d2o[u], m.t0, m.inv_delta, m.tmax, m.nb, bo[u], fo[u]);
-                        const float2 *rowp = m.Epk + (size_t)tri_row(iu[u], j, m.L) * m.nb;
-                        vn[u] = __ldg(rowp + bn[u]); vo[u] = __ldg(rowp + bo[u]);
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < U; ++u)
-                    if (near[u]) acc += (double)(fmaf(fn[u], vn[u].y, vn[u].x) - fmaf(fo[u], vo[u].y, vo[u].x));
-            }
-        };
-        if (CULL) {
-            // rows in blocks of kBlk consecutive residues (ilo = 0): a block whose bounding sphere lies beyond the last
-            // bin centre of BOTH positions of CB_j holds only pairs whose term is exactly 0, and is skipped whole;
-            // the S threads that share a column take every S-th block
-            const int nblk = i_end < 0 ? 0 : i_end / kBlk + 1;
-            for (int b = slice; b < nblk; b += S) {
-                const float4 bl = blk4[b];
-                float dx = bl.x - xn, dy = bl.y - yn, dz = bl.z - zn;
-                const float dn = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                dx = bl.x - o.x; dy = bl.y - o.y; dz = bl.z - o.z;
-                const float dq = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                if (dn >= bl.w && dq >= bl.w) continue;
-#pragma unroll
-                for (int t = 0; t < kBlk / U; ++t)
-                    if (b * kBlk + t * U <= i_end) trip(b * kBlk + t * U, 1);
-            }
+        const int j = jlo + c0 + col;
+        float xn, yn, zn;
+        if (turn) {
+            double x0, y0, z0, x, y, z;
+            if (cb64) { x0 = X[3 * m.L + j]; y0 = Y[3 * m.L + j]; z0 = Z[3 * m.L + j]; }
+            else cb_point(m, X, Y, Z, m.L, j, x0, y0, z0);
+            rot_apply(R, x0, y0, z0, x, y, z);
+            xn = (float)x; yn = (float)y; zn = (float)z;
         } else {
-            for (int i = ilo + slice; i <= i_end; i += U * S) trip(i, S);
+            const float4 o = cb4[j];
+            xn = o.x; yn = o.y; zn = o.z;
+        }
+        const int i_end = min(split - 1, j - m.min_sep);
+        const int nblk = i_end < 0 ? 0 : i_end / kBlk + 1;
+        for (int b = slice; b < nblk; b += S) {
+            const float4 bl = blk4[b];
+            {
+                const float dx = bl.x - xn, dy = bl.y - yn, dz = bl.z - zn;
+                if (fmaf(dx, dx, fmaf(dy, dy, dz * dz)) >= bl.w) continue;
+            }
+            // U rows per trip: all distances first, then all gathers, then the sums, so that a thread has U loads in
+            // flight instead of stalling on each pair's row (the rows of near pairs come from L2, ~600 cycles away)
+            constexpr int U = 4;
+            float part = 0.0f;
+#pragma unroll
+            for (int t = 0; t < kBlk / U; ++t) {
+                const int i = b * kBlk + t * U;
+                if (i <= i_end) {
+                    float d2[U], f[U];
+                    float2 v[U];
+                    bool near[U];
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        const float4 ci = cb4[min(i + u, i_end)];
+                        const float dx = ci.x - xn, dy = ci.y - yn, dz = ci.z - zn;
+                        d2[u] = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                        near[u] = (i + u <= i_end) && d2[u] < m.far2;
+                    }
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        v[u] = make_float2(0.0f, 0.0f); f[u] = 0.0f;
+                        if (near[u]) {
+                            int bn;
+                            bin_frac(d2[u], m.t0, m.inv_delta, m.tmax, m.thmax, bn, f[u]);
+                            v[u] = __ldg(m.Epk + (size_t)tri_row(i + u, j, m.L) * m.nb + bn);
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < U; ++u) part += fmaf(f[u], v[u].y, v[u].x);
+                }
+            }
+            acc += (double)part;
+        }
+    }
+    return acc;
+}
+
+// the row line of a global transition: sum of e' over (i, j), j = j0 .. j0 + cnt - 1, at the current positions
+__device__ __forceinline__ double global_row_sum(const DevModel &m, const float4 *cb4, int i, int j0, int cnt, int tid, int nthr)
+{
+    double acc = 0.0;
+    if (cnt <= 0) return acc;
+    const float4 ci = cb4[i];
+    const int rb = tri_row(i, 0, m.L);
+    for (int q = tid; q < cnt; q += nthr) {
+        const int j = j0 + q;
+        const float4 cj = cb4[j];
+        const float dx = ci.x - cj.x, dy = ci.y - cj.y, dz = ci.z - cj.z;
+        const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+        if (d2 < m.far2) {
+            int b;
+            float f;
+            bin_frac(d2, m.t0, m.inv_delta, m.tmax, m.thmax, b, f);
+            const float2 v = __ldg(m.Epk + (size_t)(rb + j) * m.nb + b);
+            acc += (double)fmaf(f, v.y, v.x);
         }
     }
     return acc;
@@ -365,6 +500,17 @@ __device__ __forceinline__ double team_sum(double v, double *red, int warp, int 
     return tot;
 }
 
+// two sums at once
+__device__ __forceinline__ void team_sum2(double &a, double &b, double *red, int warp, int nwarps, int lane, int bar_id)
+{
+    a = warp_sum(a); b = warp_sum(b);
+    if (lane == 0) { red[warp] = a; red[kMaxWarps + warp] = b; }
+    team_bar(bar_id, nwarps * 32);
+    a = 0.0; b = 0.0;
+    for (int w = 0; w < nwarps; ++w) { a += red[w]; b += red[kMaxWarps + w]; }
+    team_bar(bar_id, nwarps * 32);
+}
+
 // largest |coordinate| of the chain's C-betas (the fp32 rounding of a coordinate, hence the error bound of dE, scales with it)
 __device__ __forceinline__ float team_extent(const float4 *cb4, int L, double *red, int tid, int nthr, int warp, int nwarps, int lane, int bar_id)
 {
@@ -401,7 +547,8 @@ __device__ __forceinline__ void team_blocks(const DevModel &m, const float4 *cb4
     }
 }
 
-// V (Eq. 3a) of the team's chain from its fp32 C-betas; every thread of the team returns the same value
+// V (Eq. 3a) of the team's chain from its fp32 C-betas: v_far (every pair at its clamped value) + the excess of the
+// near pairs; every thread of the team returns the same value
 __device__ __forceinline__ double team_full_energy(const DevModel &m, const float4 *cb4, double *red, int warp, int nwarps,
                                                    int lane, int bar_id)
 {
@@ -411,42 +558,32 @@ __device__ __forceinline__ double team_full_energy(const DevModel &m, const floa
         const float4 ci = cb4[i];
         const int rb = tri_row(i, 0, m.L);
         for (int j0 = i + m.min_sep + lane; j0 < m.L; j0 += 32 * U) {
-            float d2[U], v[U], f[U];
+            float d2[U], f[U];
             float2 g[U];
-            bool far[U];
+            float part = 0.0f;
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int j = min(j0 + 32 * u, m.L - 1);
                 const float4 cj = cb4[j];
                 const float dx = ci.x - cj.x, dy = ci.y - cj.y, dz = ci.z - cj.z;
                 d2[u] = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                far[u] = d2[u] >= m.far2;
             }
-            // far pairs take the clamped value from the compact array (coalesced in j), near pairs gather their row
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int j = j0 + 32 * u;
-                v[u] = 0.0f; g[u] = make_float2(0.0f, 0.0f); f[u] = 0.0f;
-                if (j < m.L) {
-                    if (far[u]) v[u] = __ldg(m.Elast + rb + j);
-                    else {
-                        int b;
-                        lerp_coords(d2[u], m.t0, m.inv_delta, m.tmax, m.nb, b, f[u]);
-                        g[u] = __ldg(m.Epk + (size_t)(rb + j) * m.nb + b);
-                    }
+                g[u] = make_float2(0.0f, 0.0f); f[u] = 0.0f;
+                if (j < m.L && d2[u] < m.far2) {
+                    int b;
+                    bin_frac(d2[u], m.t0, m.inv_delta, m.tmax, m.thmax, b, f[u]);
+                    g[u] = __ldg(m.Epk + (size_t)(rb + j) * m.nb + b);
                 }
             }
 #pragma unroll
-            for (int u = 0; u < U; ++u) e += (double)(far[u] ? v[u] : fmaf(f[u], g[u].y, g[u].x));
+            for (int u = 0; u < U; ++u) part += fmaf(f[u], g[u].y, g[u].x);
+            e += (double)part;
         }
     }
-    e = warp_sum(e);
-    if (lane == 0) red[warp] = e;
-    team_bar(bar_id, nwarps * 32);
-    double tot = 0.0;
-    for (int w = 0; w < nwarps; ++w) tot += red[w];
-    team_bar(bar_id, nwarps * 32);
-    return tot;
+    return m.v_far + team_sum(e, red, warp, nwarps, lane, bar_id);
 }
 
 // SG: global proposals too are evaluated speculatively, one warp per step (separate instantiations, so that neither
@@ -464,13 +601,14 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     const int warp = warp_cta - slot * W;                 // warp within the team
     const int tid = warp * 32 + lane, nthreads = W * 32, nwarps = W;
     const int bar_id = 1 + slot;
+    const int w_eff = min(a.window, L - 1);
     const int span = min(2 * a.window, L - 1);            // largest j - i of an in-window pair
     constexpr bool use_ring = RING;
 
     unsigned long long *full_bar = reinterpret_cast<unsigned long long *>(smem_raw);                 // [R]
-    volatile long long *prog = reinterpret_cast<volatile long long *>(smem_raw + 8 * (size_t)R);      // [16]
-    float *ring = reinterpret_cast<float *>(smem_raw + sweep_header_bytes(R));
-    const size_t chains_off = (sweep_header_bytes(R) + sizeof(float) * (size_t)R * a.ring_rows * m.row_stride + 15) & ~(size_t)15;
+    unsigned long long *empty_bar = full_bar + R;                                                     // [R]
+    float *ring = reinterpret_cast<float *>(smem_raw + sweep_header_bytes(R)) + (R > 0 ? kRingPadRows * m.row_stride : 0);
+    const size_t chains_off = sweep_header_bytes(R) + ring_bytes(R, a.ring_rows, m.row_stride);
 
     const long long row0 = (long long)blockIdx.x * C;
     const int nvalid = (int)min((long long)C, a.B - row0);
@@ -481,70 +619,64 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     };
 
     if (threadIdx.x == 0) {
-        for (int q = 0; q < R; ++q) mbar_init(&full_bar[q], 1);
-        for (int g = 0; g < 16; ++g) prog[g] = (g < nvalid) ? 0 : 0x7fffffffffffffffLL;
+        for (int q = 0; q < R; ++q) { mbar_init(&full_bar[q], 1); mbar_init(&empty_bar[q], (uint32_t)nvalid); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
     // ================= producer warp: stream the columns of every local sweep through the ring ===========
     if (slot == C) {
-        if (!use_ring) return;
+        if (!use_ring || lane != 0) return;
         const uint32_t row_bytes = (uint32_t)(m.row_stride * sizeof(float));
-        long long q0 = 0;                                   // running number of column j = 0 of the sweep
         int s = 0;                                          // ring slot of the next column
+        long long rev = 0;                                  // revolutions of the ring so far
         for (long long t = a.sweep_offset; t < a.sweep_offset + a.n_sweeps; ++t) {
             if (sweep_is_global(t)) continue;
             for (int j = 0; j < L; ++j) {
-                const long long q = q0 + j;
-                if (lane == 0) {                            // slot s is free once every team has passed column q - R
-                    for (;;) {
-                        long long mn = 0x7fffffffffffffffLL;
-                        for (int g = 0; g < nvalid; ++g) mn = min(mn, prog[g]);
-                        if (q - R < mn) break;
-                        __nanosleep(200);
-                    }
-                    const int i_lo = max(0, j - span), i_hi = j - m.min_sep;
-                    const int nrows = i_hi - i_lo + 1;
-                    void *bar = &full_bar[s];
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the teams' reads of the old column come first
-                    if (nrows > 0) mbar_expect_tx(bar, (uint32_t)nrows * row_bytes);
-                    else mbar_arrive(bar);
-                    // one lane issues the copies of the column: the operands of a bulk copy live in uniform registers
-                    for (int i = i_lo; i <= i_hi; ++i)
-                        tma_bulk_g2s(ring + ((size_t)s * a.ring_rows + (i - j + span)) * m.row_stride,
-                                     m.Epl + (size_t)tri_row(i, j, L) * m.row_stride, row_bytes, bar);
+                // slot s is free once every team has arrived on its empty barrier for the column it held before
+                if (rev > 0) mbar_wait(&empty_bar[s], (uint32_t)((rev - 1) & 1));
+                const int nrows = min(span, j) - m.min_sep + 1;   // rows j - i = min_sep .. min(span, j): contiguous in Ebd
+                void *bar = &full_bar[s];
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the teams' reads of the old column come first
+                if (nrows > 0) {
+                    mbar_expect_tx(bar, (uint32_t)nrows * row_bytes);
+                    tma_bulk_g2s(ring + (size_t)s * a.ring_rows * m.row_stride, m.Ebd + (size_t)j * m.band_rows * m.row_stride,
+                                 (uint32_t)nrows * row_bytes, bar);
+                } else {
+                    mbar_arrive(bar);
                 }
-                __syncwarp();
-                if (++s == R) s = 0;
+                if (++s == R) { s = 0; ++rev; }
             }
-            q0 += L;
         }
         return;
     }
     if (slot >= nvalid) return;
 
     // ================= team: one chain =====================================================================
-    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L, a.cb64);
+    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L, a.cb64, a.nspec, a.wpts);
     constexpr bool cb64 = CB64;
     const int na = cb64 ? 4 : 3;                            // atoms per residue kept in fp64
     double *X = reinterpret_cast<double *>(cbase), *Y = X + na * L, *Z = Y + na * L;
-    double *red = Z + na * L + (cb64 ? 0 : (L & 1)), *b_cd = red + kMaxWarps, *b_sd = b_cd + kDrawBatch, *b_lu = b_sd + kDrawBatch;
-    double *rot_s = b_lu + kDrawBatch, *sp_dE = rot_s + 12 * kMaxSpec;
-    float4 *cb4 = reinterpret_cast<float4 *>(sp_dE + kMaxSpec);
+    double *red = Z + na * L + ((3 * na * L) & 1), *b_cd = red + 2 * kMaxWarps, *b_sd = b_cd + kDrawBatch, *b_lu = b_sd + kDrawBatch;
+    double *rot_s = b_lu + kDrawBatch, *sp_new = rot_s + 12 * kMaxSpec, *sp_T = sp_new + kMaxSpec;
+    float4 *cb4 = reinterpret_cast<float4 *>(sp_T + kMaxSpec);
     float4 *blk4 = cb4 + L;
-    float *s = reinterpret_cast<float *>(blk4 + (L + kBlk - 1) / kBlk);
+    float4 *cbn = blk4 + (L + kBlk - 1) / kBlk;
+    float *s = reinterpret_cast<float *>(cbn + (size_t)a.nspec * a.wpts);
     float *b_sp = s + n;
-    int *sp_acc = reinterpret_cast<int *>(b_sp + kDrawBatch);
 
     const long long row = row0 + slot;
     const unsigned long long chain = (unsigned long long)(a.chain_offset + row);
 
     for (int q = tid; q < n; q += nthreads) s[q] = a.states[row * n + q];
     team_bar(bar_id, nthreads);
+    // the row term of residue i in a local table address (see LocalTab)
+    auto row_term = [&](int i) -> float {
+        return __int_as_float(use_ring ? -i * m.row_stride * 4 : (int)(tri_base(i, L) * m.nb * 8));
+    };
     if (warp == 0)
         nerf_build_warp(m, s, lane, [&](int res, int at, double x, double y, double z) {
-            if (at == 3) cb4[res] = make_float4((float)x, (float)y, (float)z, 0.0f);
+            if (at == 3) cb4[res] = make_float4((float)x, (float)y, (float)z, row_term(res));
             if (at < na) { const int f = at * L + res; X[f] = x; Y[f] = y; Z[f] = z; }
         });
     team_bar(bar_id, nthreads);
@@ -557,16 +689,17 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     const int gshift = a.lanes_per_step == 8 ? 3 : (a.lanes_per_step == 16 ? 4 : 5);
     const int gl = 1 << gshift, gpw = 32 >> gshift;
     const int grp = lane >> gshift, glane = lane & (gl - 1);
-    int nspec = max(1, min(min(nwarps * gpw, kMaxSpec), a.spec_local > 0 ? a.spec_local : kMaxSpec));
-    // a pass may not reach beyond what the ring can hold next to the window (else the team would wait for a column
-    // whose slot it still occupies itself)
-    if (use_ring) nspec = max(1, min(nspec, 2 * (R - min(a.window, L - 1) - 2) - 1));
-    const int draw_warp_u = nwarps > 1 ? 1 : 0;              // the warp that draws the uniforms of the accept test
-    long long q0 = 0;                                        // running column number of j = 0 (local sweeps)
+    const int nspec = a.nspec;
+    // ring bookkeeping of this team: the slot of column 0 of the current local sweep, the columns it has waited for and
+    // the columns it has released
+    int slot_j0 = 0;                                         // ring slot of column 0 of this sweep
     int seen_slot = R - 1;                                   // ring slot and phase parity of the last column waited for
     uint32_t seen_par = 1;
-    RowSource rs;
-    rs.ring = use_ring ? ring : nullptr; rs.ring_cols = R; rs.ring_rows = a.ring_rows; rs.span = span; rs.slot0 = 0;
+    int dead_slot = 0;                                       // ring slot of the next column to release
+    LocalTab tb;
+    tb.base = use_ring ? reinterpret_cast<const unsigned char *>(ring) : reinterpret_cast<const unsigned char *>(m.Epk);
+    tb.ring_cols = R; tb.ring_rows = a.ring_rows; tb.min_sep = m.min_sep; tb.stride4 = m.row_stride * 4; tb.nb8 = m.nb * 8;
+    tb.slot_c = 0; tb.c_ref = 0;
 
     // the bond the torsion k turns about: phi_c N->CA, psi_c CA->C
     auto step_rot = [&](int k, int bi) -> Rot {
@@ -588,19 +721,19 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 X[f] = x; Y[f] = y; Z[f] = z;
             }
             double x, y, z;
-            if (cb64 && (res > c || (k & 1) == 0)) {         // the stored C-beta turns with its residue
+            if (cb64) {                                      // the stored C-beta turns with its residue
                 const int f = 3 * L + res;
                 rot_apply(R_, X[f], Y[f], Z[f], x, y, z);
                 X[f] = x; Y[f] = y; Z[f] = z;
             } else {
                 cb_point(m, X, Y, Z, L, res, x, y, z);
             }
-            cb4[res] = make_float4((float)x, (float)y, (float)z, 0.0f);
+            cb4[res] = make_float4((float)x, (float)y, (float)z, row_term(res));
         }
     };
 
     for (long long t = a.sweep_offset; t < a.sweep_offset + a.n_sweeps; ++t) {
-        const bool is_global = sweep_is_global(t);
+        const bool gp = sweep_is_global(t);                  // proposals judged on all pairs (Eq. 1) or on the window (Eq. 2)
         double T;
         if (a.per_chain_T) T = (double)a.per_chain_T[row];
         else if (a.t_start == a.t_end || a.ramp_sweeps <= 1 || t <= 0) T = a.t_start;
@@ -612,9 +745,11 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
             sigma_t = (t >= a.ramp_sigma - 1) ? a.sigma_end
                                               : a.sigma_start + (a.sigma_end - a.sigma_start) * ((double)t / (double)(a.ramp_sigma - 1));
         int seen_rel = -1;                                   // last column of this sweep the team has waited for
-        const int slot_j0 = (seen_slot + 1 == R) ? 0 : seen_slot + 1;   // ring slot of column 0 of this sweep
+        int dead_rel = 0;                                    // columns < dead_rel of this sweep have been released (tid 0)
+        const double guard = (gp ? a.guard_global : a.guard_local) * ext_scale * invT;
+        double S_base = 0.0;                                 // S_old of step k - 1 for the current state (every thread holds it)
 
-        if (is_global) {                                     // the local sweeps moved everything: fresh culling blocks
+        if (gp) {                                            // the local sweeps moved everything: fresh culling blocks
             team_blocks(m, cb4, blk4, 0, tid, nthreads);
             team_bar(bar_id, nthreads);
         }
@@ -623,6 +758,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
             // ---- a1/a2: draws of the next 64 steps, two per lane (R5-R7) ----------------------------------
             if (k >= batch_end) {
                 batch_start = k; batch_end = min(n, k + kDrawBatch);
+                const int draw_warp_u = nwarps > 1 ? 1 : 0;   // the warp that draws the uniforms of the accept test
                 if (warp == 0 || warp == draw_warp_u) {
 #pragma unroll 1
                     for (int bi = lane; bi < kDrawBatch; bi += 32) {
@@ -661,169 +797,198 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 }
                 team_bar(bar_id, nthreads);
             }
-            if (is_global && !SG) {
-                // ======== one proposal, evaluated by the whole team ========================================
+            // ---- a pass: S proposals, group r evaluating step k + r against the current state -------------------
+            // local sweeps: groups of gl lanes; global sweeps: SG = one warp per step, else one step by the whole team
+            const bool teamwide = gp && !SG;
+            const int S = teamwide ? 1 : min(gp ? min(nwarps, kMaxSpec) : nspec, batch_end - k);
+            double my_new = 0.0, my_T = 0.0;                 // S_new and T of step k + lane, lane < S (filled below)
+            if (teamwide) {
+                // ======== one proposal, evaluated by the whole team (a3/a5/a6) =================================
                 const int bi = k - batch_start;
                 const int split = (k >> 1) + (k & 1);
                 const bool inert = (k == 0) || (k == n - 1);
-                double dE = 0.0;
+                double p_new = 0.0, p_T = 0.0;
+                Rot Rk;
                 if (!inert) {
-                    // ---- a3/a5/a6: turn the right-hand side about the flipped bond, cross pairs, reduction ------
-                    double acc;
-                    {
-                        const Rot Rk = step_rot(k, bi);
-                        if (tid == 0) {                       // kept in shared memory for the commit, not in registers
+                    Rk = step_rot(k, bi);
+                    if (tid == 0) {                           // kept in shared memory for the commit, not in registers
 #pragma unroll
-                            for (int q = 0; q < 9; ++q) rot_s[q] = Rk.r[q];
+                        for (int q = 0; q < 9; ++q) rot_s[q] = Rk.r[q];
 #pragma unroll
-                            for (int q = 0; q < 3; ++q) rot_s[9 + q] = Rk.t[q];
-                        }
-                        acc = warp_sum(cross_pairs_dE<false, true>(m, rs, cb4, blk4, X, Y, Z, cb64, Rk, 0, split, L - 1, tid, nthreads));
+                        for (int q = 0; q < 3; ++q) rot_s[9 + q] = Rk.t[q];
                     }
-                    if (lane == 0) red[warp] = acc;
-                    team_bar(bar_id, nthreads);
-                    for (int w = 0; w < nwarps; ++w) dE += red[w];
+                    p_new = global_cols_sum(m, cb4, blk4, X, Y, Z, cb64, true, Rk, split, split, L - 1, tid, nthreads);
                 }
-                // ---- a7: Metropolis test, accept iff log u <= -dE / T   (Eq. 1a, R14) ---------------------
-                // exact-decision guard (R24): a gap inside the fp32 error bound of dE is decided by the fp64 path
-                bool exact = false;
-                if (!inert && fabs(b_lu[bi] + dE * invT) < a.guard_global * ext_scale * invT) {
-                    team_bar(bar_id, nthreads);                      // every thread has read red[]
-                    dE = team_sum(exact_dE_partial(m, X, Y, Z, cb64 ? 1 : 0, k, b_cd[bi], b_sd[bi], 0, L - 1, tid, nthreads),
-                                  red, warp, nwarps, lane, bar_id);
-                    exact = true;
+                if (k & 1) {                                  // the split moved: column c leaves, row c enters
+                    const int c = k >> 1;
+                    p_T = global_row_sum(m, cb4, c, c + m.min_sep, L - c - m.min_sep, tid, nthreads)
+                        - global_cols_sum(m, cb4, blk4, X, Y, Z, cb64, false, Rk, c, c, c, tid, nthreads);
                 }
-                const bool accept = exact ? (b_lu[bi] <= -dE / T) : (b_lu[bi] <= -dE * invT);
-                if (tid == 0) {
-                    const long long q = (t - a.sweep_offset) * n + k;
-                    if (q < a.trace_steps) {
-                        const size_t z = (size_t)row * a.trace_steps + q;
-                        if (a.trace_prop) a.trace_prop[z] = b_sp[bi];
-                        if (a.trace_dE) a.trace_dE[z] = dE;
-                        if (a.trace_acc) a.trace_acc[z] = (accept ? 1 : 0) | (exact ? 2 : 0);
-                    }
-                }
-                if (accept) {
-                    ++acc_g;
-                    if (tid == 0) s[k] = b_sp[bi];
-                    if (!inert) {
-                        Rot Rc;
-#pragma unroll
-                        for (int q = 0; q < 9; ++q) Rc.r[q] = rot_s[q];
-#pragma unroll
-                        for (int q = 0; q < 3; ++q) Rc.t[q] = rot_s[9 + q];
-                        commit(Rc, k);
-                        team_bar(bar_id, nthreads);
-                        team_blocks(m, cb4, blk4, (k >> 1) / kBlk, tid, nthreads);
-                    }
-                }
-                team_bar(bar_id, nthreads);
-                ++k;
+                team_sum2(p_new, p_T, red, warp, nwarps, lane, bar_id);
+                my_new = p_new; my_T = p_T;
             } else {
-                // ======== up to nspec proposals, group r evaluating step k + r against the current state ===
-                // (a global sweep in speculative mode: the groups are whole warps and the pairs are all straddling ones)
-                const bool gp = SG && is_global;
-                const int gl_x = gp ? 32 : gl, gpw_x = gp ? 1 : gpw;
-                const int grp_x = gp ? 0 : grp, glane_x = gp ? lane : glane;
-                const int S = min(gp ? min(nwarps, kMaxSpec) : nspec, batch_end - k);
                 if (use_ring && !gp) {
                     // columns left of the window centre are dead for this chain; wait for the ones the pass needs
-                    if (tid == 0) prog[slot] = q0 + (k >> 1);
+                    const int c_now = k >> 1;
+                    if (tid == 0)
+                        while (dead_rel < c_now) {
+                            mbar_arrive(&empty_bar[dead_slot]);
+                            ++dead_rel;
+                            if (++dead_slot == R) dead_slot = 0;
+                        }
                     const int need = min(L - 1, ((k + S - 1) >> 1) + a.window);
                     while (seen_rel < need) {
                         ++seen_rel;
                         if (++seen_slot == R) { seen_slot = 0; seen_par ^= 1u; }
                         mbar_wait(&full_bar[seen_slot], seen_par);
                     }
+                    tb.c_ref = c_now;
+                    tb.slot_c = slot_j0 + c_now;
+                    if (tb.slot_c >= R) tb.slot_c %= R;
                 }
-                const int r = warp * gpw_x + grp_x;
+                const int r = gp ? warp : warp * gpw + grp;
+                const int gl_x = gp ? 32 : gl, glane_x = gp ? lane : glane;
                 const bool active = r < S;
-                const int kk = k + r, bi = kk - batch_start;
+                const int kk = k + r, bi = min(kk, batch_end - 1) - batch_start;
                 const bool inert = (kk == 0) || (kk == n - 1);
-                double dE = 0.0;
-                Rot Rk;
-                if (active && !inert) {
-                    const int c = kk >> 1, split = c + (kk & 1);
-                    Rk = step_rot(kk, bi);
-                    const int ilo = gp ? 0 : max(0, c - a.window), jhi = gp ? L - 1 : min(L - 1, c + a.window);
-                    // ---- a4/a5: in-window cross pairs (Eq. 3b), or all of them (Eq. 3a) ------------------------
-                    if (gp) {
-                        dE = cross_pairs_dE<false, true>(m, rs, cb4, blk4, X, Y, Z, cb64, Rk, 0, split, L - 1, lane, 32);
-                    } else {
-                        if (RING) {
-                            rs.slot0 = slot_j0 + split;
-                            if (rs.slot0 >= R) rs.slot0 %= R;
+                const int c = kk >> 1, split = c + (kk & 1);
+                double p_new = 0.0, p_T = 0.0;
+                if (gp) {
+                    // ---- a5: all straddling pairs (Eq. 3a), one warp ---------------------------------------------
+                    if (active) {
+                        Rot Rk;
+                        if (!inert) {
+                            Rk = step_rot(kk, bi);
+                            if (lane == 0) {
+#pragma unroll
+                                for (int q = 0; q < 9; ++q) rot_s[12 * r + q] = Rk.r[q];
+#pragma unroll
+                                for (int q = 0; q < 3; ++q) rot_s[12 * r + 9 + q] = Rk.t[q];
+                            }
+                            p_new = global_cols_sum(m, cb4, blk4, X, Y, Z, cb64, true, Rk, split, split, L - 1, lane, 32);
                         }
-                        dE = cross_pairs_dE<RING, false>(m, rs, cb4, blk4, X, Y, Z, cb64, Rk, ilo, split, jhi, glane_x, gl_x);
+                        if (kk & 1)
+                            p_T = global_row_sum(m, cb4, c, c + m.min_sep, L - c - m.min_sep, lane, 32)
+                                - global_cols_sum(m, cb4, blk4, X, Y, Z, cb64, false, Rk, c, c, c, lane, 32);
+                    }
+                } else {
+                    // ---- a3/a4: in-window straddling pairs (Eq. 3b) ------------------------------------------------
+                    const int ilo = max(0, c - w_eff), jhi = min(L - 1, c + w_eff);
+                    const int nI = split - ilo, nJ = jhi - split + 1;
+                    float4 *cbn_r = cbn + (size_t)min(r, nspec - 1) * a.wpts;
+                    if (active && !inert) {
+                        const Rot Rk = step_rot(kk, bi);
+                        if (glane_x == 0) {
+#pragma unroll
+                            for (int q = 0; q < 9; ++q) rot_s[12 * r + q] = Rk.r[q];
+#pragma unroll
+                            for (int q = 0; q < 3; ++q) rot_s[12 * r + 9 + q] = Rk.t[q];
+                        }
+                        for (int jj = glane_x; jj < nJ; jj += gl_x) {
+                            const int j = split + jj;
+                            double x0, y0, z0, x, y, z;
+                            if (cb64) { x0 = X[3 * L + j]; y0 = Y[3 * L + j]; z0 = Z[3 * L + j]; }
+                            else cb_point(m, X, Y, Z, L, j, x0, y0, z0);
+                            rot_apply(Rk, x0, y0, z0, x, y, z);
+                            cbn_r[jj] = make_float4((float)x, (float)y, (float)z, __int_as_float(col_term<RING>(tb, j)));
+                        }
+                    }
+                    __syncwarp();
+                    if (active) {
+                        if (!inert) p_new = (double)local_new_sum<RING>(m, tb, cb4, cbn_r, ilo, split, nI, nJ, glane_x, gl_x);
+                        p_T = (double)local_transition<RING>(m, tb, cb4, kk, w_eff, glane_x, gl_x);
                     }
                 }
                 // ---- a6: reduction over the group's lanes (every lane of the warp takes part) ----------------
-                for (int d = gl_x >> 1; d > 0; d >>= 1) dE += __shfl_xor_sync(0xffffffffu, dE, d);
-                if (active && glane_x == 0) {
-                    sp_dE[r] = dE;
-                    const double gd = (gp ? a.guard_global : a.guard_local) * ext_scale * invT;
-                    // Eq. 2a, R14; 2 = the gap is inside the fp32 error bound of dE: decided below by the fp64 path (R24)
-                    sp_acc[r] = (!inert && fabs(b_lu[bi] + dE * invT) < gd) ? 2 : ((b_lu[bi] <= -dE * invT) ? 1 : 0);
-                    if (!inert) {
-#pragma unroll
-                        for (int q = 0; q < 9; ++q) rot_s[12 * r + q] = Rk.r[q];
-#pragma unroll
-                        for (int q = 0; q < 3; ++q) rot_s[12 * r + 9 + q] = Rk.t[q];
-                    }
+                for (int d = gl_x >> 1; d > 0; d >>= 1) {
+                    p_new += __shfl_xor_sync(0xffffffffu, p_new, d);
+                    p_T += __shfl_xor_sync(0xffffffffu, p_T, d);
                 }
+                if (active && glane_x == 0) { sp_new[r] = p_new; sp_T[r] = p_T; }
                 team_bar(bar_id, nthreads);
-                int rsel = 0;                                 // first accepted step of the pass
-                bool any_exact = false;
-                while (rsel < S) {
-                    int f = sp_acc[rsel];                     // the same value in every thread of the team
-                    if (f == 2) {
-                        const int kx = k + rsel, bx = kx - batch_start, cx = kx >> 1;
-                        const double dx = team_sum(exact_dE_partial(m, X, Y, Z, cb64 ? 1 : 0, kx, b_cd[bx], b_sd[bx],
-                                                                    gp ? 0 : max(0, cx - a.window), gp ? L - 1 : min(L - 1, cx + a.window),
-                                                                    tid, nthreads), red, warp, nwarps, lane, bar_id);
-                        f = 2 | ((b_lu[bx] <= -dx / T) ? 1 : 0);
-                        if (tid == 0) { sp_dE[rsel] = dx; sp_acc[rsel] = f; }   // after team_sum's barriers: every thread has read the 2
-                        any_exact = true;
-                    }
-                    if (f & 1) break;
-                    ++rsel;
-                }
-                if (any_exact) team_bar(bar_id, nthreads);    // the rewritten entries are read by the tracing threads
-                const int nstand = (rsel < S) ? rsel + 1 : S; // steps whose result stands
-                if (tid < nstand) {
-                    const long long q = (t - a.sweep_offset) * n + k + tid;
-                    if (q < a.trace_steps) {
-                        const size_t z = (size_t)row * a.trace_steps + q;
-                        if (a.trace_prop) a.trace_prop[z] = b_sp[k + tid - batch_start];
-                        if (a.trace_dE) a.trace_dE[z] = sp_dE[tid];
-                        if (a.trace_acc) a.trace_acc[z] = (unsigned char)sp_acc[tid];
-                    }
-                }
-                if (rsel < S) {
-                    // ---- a7: commit the accepted step --------------------------------------------------------
-                    const int kc = k + rsel;
-                    if (gp) ++acc_g; else ++acc_l;
-                    if (tid == 0) s[kc] = b_sp[kc - batch_start];
-                    if (kc != 0 && kc != n - 1) {
-                        Rot Rc;
-#pragma unroll
-                        for (int q = 0; q < 9; ++q) Rc.r[q] = rot_s[12 * rsel + q];
-#pragma unroll
-                        for (int q = 0; q < 3; ++q) Rc.t[q] = rot_s[12 * rsel + 9 + q];
-                        commit(Rc, kc);
-                        if (gp) {
-                            team_bar(bar_id, nthreads);
-                            team_blocks(m, cb4, blk4, (kc >> 1) / kBlk, tid, nthreads);
-                        }
-                    }
-                }
-                team_bar(bar_id, nthreads);
-                k += nstand;
+                if (lane < S) { my_new = sp_new[lane]; my_T = sp_T[lane]; }
             }
+            // ---- a7: Metropolis tests in step order; lane r holds step k + r ---------------------------------------------
+            // S_old(k + r) = S_base + T(k) + ... + T(k + r)  (inclusive prefix over the lanes)
+            double pre = my_T;
+#pragma unroll
+            for (int d = 1; d < kMaxSpec; d <<= 1) {
+                const double v = __shfl_up_sync(0xffffffffu, pre, d);
+                if (lane >= d) pre += v;
+            }
+            const double s_old = S_base + pre;
+            const int kq = k + lane;                          // this lane's step (meaningful for lane < S)
+            const int bq = min(kq, batch_end - 1) - batch_start;
+            const bool inert_q = (kq == 0) || (kq == n - 1);
+            double dE = inert_q ? 0.0 : my_new - s_old;
+            const double lu = b_lu[bq];
+            // exact-decision guard (R24): a gap inside the fp32 error bound of dE is decided by the fp64 path
+            const bool unc = lane < S && !inert_q && fabs(lu + dE * invT) < guard;
+            bool acc = lane < S && (lu <= -dE * invT);        // Eq. 1a/2a, R14
+            const unsigned m_unc = __ballot_sync(0xffffffffu, unc);
+            unsigned m_go = __ballot_sync(0xffffffffu, acc || unc);
+            unsigned m_exact = 0;
+            int rsel = S;                                     // first accepted step of the pass
+            while (m_go) {
+                const int r0 = __ffs(m_go) - 1;
+                if (!((m_unc >> r0) & 1u)) { rsel = r0; break; }
+                const int kx = k + r0, bx = kx - batch_start, cx = kx >> 1;
+                const double dx = team_sum(exact_dE_partial(m, X, Y, Z, cb64 ? 1 : 0, kx, b_cd[bx], b_sd[bx],
+                                                            gp ? 0 : max(0, cx - w_eff), gp ? L - 1 : min(L - 1, cx + w_eff),
+                                                            tid, nthreads), red, warp, nwarps, lane, bar_id);
+                const bool ax = b_lu[bx] <= -dx / T;
+                if (lane == r0) { dE = dx; acc = ax; }
+                m_exact |= 1u << r0;
+                if (ax) { rsel = r0; break; }
+                m_go &= ~(1u << r0);
+            }
+            const int nstand = (rsel < S) ? rsel + 1 : S;     // steps whose result stands
+            if (warp == 0 && lane < nstand) {
+                const long long q = (t - a.sweep_offset) * n + kq;
+                if (q < a.trace_steps) {
+                    const size_t z = (size_t)row * a.trace_steps + q;
+                    if (a.trace_prop) a.trace_prop[z] = b_sp[bq];
+                    if (a.trace_dE) a.trace_dE[z] = dE;
+                    if (a.trace_acc) a.trace_acc[z] = (unsigned char)((lane == rsel ? 1 : 0) | (((m_exact >> lane) & 1u) ? 2 : 0));
+                }
+            }
+            // S_old carried to the next pass: an accepted proposal's S_new is the S_old of its step for the new state
+            // (an inert one moves nothing); without an accept, the S_old of the last step evaluated
+            {
+                const int src = (rsel < S) ? rsel : S - 1;
+                const bool take_new = (rsel < S) && !((k + rsel == 0) || (k + rsel == n - 1));
+                S_base = __shfl_sync(0xffffffffu, take_new ? my_new : s_old, src);
+            }
+            if (rsel < S) {
+                // ---- commit the accepted step --------------------------------------------------------
+                const int kc = k + rsel;
+                if (gp) ++acc_g; else ++acc_l;
+                if (tid == 0) s[kc] = b_sp[kc - batch_start];
+                if (kc != 0 && kc != n - 1) {
+                    Rot Rc;
+#pragma unroll
+                    for (int q = 0; q < 9; ++q) Rc.r[q] = rot_s[12 * rsel + q];
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) Rc.t[q] = rot_s[12 * rsel + 9 + q];
+                    commit(Rc, kc);
+                    if (gp) {
+                        team_bar(bar_id, nthreads);
+                        team_blocks(m, cb4, blk4, (kc >> 1) / kBlk, tid, nthreads);
+                    }
+                }
+            }
+            team_bar(bar_id, nthreads);
+            k += nstand;
         }
-        if (!is_global) {
-            q0 += L;
-            if (use_ring && tid == 0) prog[slot] = q0;       // every column of this sweep is dead for this chain
+        if (!gp && use_ring) {
+            // every column of this sweep is dead for this chain
+            if (tid == 0)
+                while (dead_rel < L) {
+                    mbar_arrive(&empty_bar[dead_slot]);
+                    ++dead_rel;
+                    if (++dead_slot == R) dead_slot = 0;
+                }
+            slot_j0 = (slot_j0 + L) % R;
         }
         // ---- a9: book-keeping at the sweep end ----------------------------------------------------
         e_end = team_full_energy(m, cb4, red, warp, nwarps, lane, bar_id);

@@ -378,7 +378,7 @@ def test_large_chain_wide_window_and_size_limit(amh, orc, torch, synth):
     ra = g2.run(a, 3, trace_steps=3 * 2 * L2, **wide); rb = g2.run(b, 3, trace_steps=3 * 2 * L2, **glob)
     assert g2.launch_info(6, 1000)["ring_cols"] == 0
     assert torch.equal(ra["trace_acc"] & 1, rb["trace_acc"] & 1) and torch.equal(a, b)
-    assert np.abs(ra["trace_dE"].cpu().numpy() - rb["trace_dE"].cpu().numpy()).max() < 1e-9
+    assert np.abs(ra["trace_dE"].cpu().numpy() - rb["trace_dE"].cpu().numpy()).max() < 1e-3   # two fp32 summation orders
     _follow_check(m2, s1, ra, 3 * 2 * L2, **wide)
     # (iii)
     with pytest.raises(amh.AMHError) as ex:
