@@ -77,7 +77,7 @@ typedef struct {
     int    spec_local;                           /* local proposals evaluated per pass (results consumed in order up to the
                                                     first accept: same trajectory); 0 = as many as the team has lane groups,
                                                     at most 16 */
-    int    lanes_per_step;                       /* lanes that share one local proposal: 0 = choose; else 8, 16 or 32 */
+    int    lanes_per_step;                       /* lanes that share one local proposal: 0 = choose; else 4, 8, 16 or 32 */
     int    spec_global;                          /* global proposals: 1 = one warp per step, speculative like the local ones;
                                                     0 = one step at a time by the whole team; -1 = choose */
     int    chains_per_cta;                       /* chains sharing one CTA and its table ring: 0 = choose; else 1..15,

@@ -71,8 +71,8 @@ static amh_status check_launch_options(const amh_launch_options &o)
         return fail(AMH_ERR_INVALID_ARG, "launch options: chains_per_cta = %d outside [0, %d]", cc, amh::kMaxChains);
     if (w > 0 && cc > 0 && w * cc > amh::kMaxTeamWarps)
         return fail(AMH_ERR_INVALID_ARG, "launch options: warps_per_chain * chains_per_cta = %d > %d", w * cc, amh::kMaxTeamWarps);
-    if (!(o.lanes_per_step == 0 || o.lanes_per_step == 8 || o.lanes_per_step == 16 || o.lanes_per_step == 32))
-        return fail(AMH_ERR_INVALID_ARG, "launch options: lanes_per_step = %d not in {0, 8, 16, 32}", o.lanes_per_step);
+    if (!(o.lanes_per_step == 0 || o.lanes_per_step == 4 || o.lanes_per_step == 8 || o.lanes_per_step == 16 || o.lanes_per_step == 32))
+        return fail(AMH_ERR_INVALID_ARG, "launch options: lanes_per_step = %d not in {0, 4, 8, 16, 32}", o.lanes_per_step);
     if (o.spec_local < 0 || o.spec_local > amh::kMaxSpec)
         return fail(AMH_ERR_INVALID_ARG, "launch options: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxSpec);
     return AMH_OK;
@@ -196,10 +196,10 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     m.cbC = m.loc[3][2] / m.loc[2][1];
 
     if (n_bins > (1 << 20)) { delete c; return fail(AMH_ERR_UNSUPPORTED, "amh_create: n_bins = %d > 2^20", n_bins); }
-    if (amh::sweep_smem_bytes(n_res, 1, 0, 0, 0, 0, 1, 1) > (size_t)c->max_smem) {
+    if (amh::sweep_smem_bytes(n_res, 1, 1, 0, 0, 0, 0, 1, 1) > (size_t)c->max_smem) {
         delete c;
         return fail(AMH_ERR_UNSUPPORTED, "amh_create: L = %d needs %zu B of shared memory per chain, device allows %d",
-                    n_res, amh::sweep_smem_bytes(n_res, 1, 0, 0, 0, 0, 1, 1), c->max_smem);
+                    n_res, amh::sweep_smem_bytes(n_res, 1, 1, 0, 0, 0, 0, 1, 1), c->max_smem);
     }
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -368,16 +368,16 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
         return w_eff + 3 + (ns + 1) / 2 + (C > 1 ? 4 : 0);
     };
     sh.cb64 = 1;
-    auto fits = [&](int C, int R, int ns) { return amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride, sh.cb64, ns, sh.wpts) <= budget; };
+    auto warps_for = [&](int C_) {
+        const int W = c->lopt.warps_per_chain;
+        return W > 0 ? std::max(1, std::min(W, amh::kMaxTeamWarps / C_)) : std::max(1, std::min(amh::kMaxTeamWarps / C_, 8));
+    };
+    auto fits = [&](int C, int R, int ns) { return amh::sweep_smem_bytes(L, C, warps_for(C), R, sh.ring_rows, c->m.row_stride, sh.cb64, ns, sh.wpts) <= budget; };
     // chains per CTA: spread the batch over the SMs (one CTA each) and keep as many teams resident as shared memory
     // allows; the ring is added only when it fits beside them (warps in flight are worth more than the ring)
     int C = c->lopt.chains_per_cta;
     const bool auto_c = C <= 0;
     if (auto_c) C = (int)std::min<long long>(7, std::max<long long>(1, (B + c->n_sm - 1) / c->n_sm));    // 7 x 2 warps + producer
-    auto warps_for = [&](int C_) {
-        const int W = c->lopt.warps_per_chain;
-        return W > 0 ? std::max(1, std::min(W, amh::kMaxTeamWarps / C_)) : std::max(1, std::min(amh::kMaxTeamWarps / C_, 8));
-    };
     if (auto_c) {
         // the fp64 C-betas (24 L bytes per chain) are dropped before a chain is (they can be rebuilt from N, CA, C)
         if (!fits(C, 0, spec_for(warps_for(C)))) sh.cb64 = 0;
@@ -400,7 +400,7 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
     if (R > 0) ns = std::max(1, std::min(ns, 2 * (R - w_eff - 2) - 1));
     sh.C = C; sh.W = W; sh.R = R; sh.nspec = ns;
     if (R == 0) sh.ring_rows = 0;
-    sh.smem = amh::sweep_smem_bytes(L, C, R, sh.ring_rows, c->m.row_stride, sh.cb64, ns, sh.wpts);
+    sh.smem = amh::sweep_smem_bytes(L, C, W, R, sh.ring_rows, c->m.row_stride, sh.cb64, ns, sh.wpts);
     return sh;
 }
 

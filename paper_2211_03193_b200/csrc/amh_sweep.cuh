@@ -39,6 +39,12 @@
 #include "amh_device.cuh"
 
 namespace amh {
+#ifndef AMH_UL
+#define AMH_UL 3
+#endif
+#ifndef AMH_UG
+#define AMH_UG 4
+#endif
 
 struct RunArgs {
     float *states;
@@ -89,7 +95,7 @@ constexpr int kRingPadRows = 4;          // rows in front of the first ring slot
 //   float4 blk4[ceil(L/8)]       bounding spheres of 8-residue blocks (culling in the global phase)
 //   float4 cbn[nspec][wpts]      the turned C-betas of the local proposals of a pass; .w = the column's term
 //   float  s[n], b_sp[64]
-__host__ __device__ inline size_t chain_smem_bytes(int L, int cb64, int nspec, int wpts)
+__host__ __device__ inline size_t chain_smem_bytes(int L, int cb64, int nspec, int wpts, int W)
 {
     size_t doubles = (cb64 ? 12 : 9) * (size_t)L;
     doubles += doubles & 1;                                  // float4 arrays on 16 bytes
@@ -108,9 +114,9 @@ __host__ __device__ inline size_t ring_bytes(int ring_cols, int ring_rows, int r
     return (sizeof(float) * ((size_t)ring_cols * ring_rows + kRingPadRows) * row_stride + 15) & ~(size_t)15;
 }
 
-__host__ __device__ inline size_t sweep_smem_bytes(int L, int C, int ring_cols, int ring_rows, int row_stride, int cb64, int nspec, int wpts)
+__host__ __device__ inline size_t sweep_smem_bytes(int L, int C, int W, int ring_cols, int ring_rows, int row_stride, int cb64, int nspec, int wpts)
 {
-    return sweep_header_bytes(ring_cols) + ring_bytes(ring_cols, ring_rows, row_stride) + (size_t)C * chain_smem_bytes(L, cb64, nspec, wpts);
+    return sweep_header_bytes(ring_cols) + ring_bytes(ring_cols, ring_rows, row_stride) + (size_t)C * chain_smem_bytes(L, cb64, nspec, wpts, W);
 }
 
 // ---- PTX: mbarrier, TMA bulk copy, named barriers ----------------------------------------------------
@@ -181,7 +187,8 @@ __device__ __forceinline__ Rot rot_about(double ax, double ay, double az, double
 }
 
 // C-beta of residue `res` from its own N, CA, C (fp64): ideal geometry makes it a fixed combination of them (R3)
-__device__ __forceinline__ void cb_point(const DevModel &m, const double *X, const double *Y, const double *Z, int L, int res,
+template <class Model>
+__device__ __forceinline__ void cb_point(const Model &m, const double *X, const double *Y, const double *Z, int L, int res,
                                          double &x, double &y, double &z)
 {
     const double ax = X[L + res], ay = Y[L + res], az = Z[L + res];                                  // CA
@@ -194,7 +201,8 @@ __device__ __forceinline__ void cb_point(const DevModel &m, const double *X, con
 
 // bin index b and fraction f of R8's interpolation at squared distance d2: t = (d - c0) / delta clamped to
 // [0, nb-1], b <= t <= b + 1, b <= nb - 2, f = t - b.
-//   d = sqrt.approx.f32(d2): one MUFU instruction, maximum relative error 2^-23 (PTX ISA); d2 = 0 gives 0.
+//   d = sqrt.approx.ftz.f32(d2): one MUFU instruction, maximum relative error 2^-23 (PTX ISA); d2 = 0 (or a
+//   subnormal: coincident atoms) gives 0.
 //   b = round-to-nearest-even(t - 1/2), read off the low mantissa bits of (t - 1/2) + 1.5 * 2^23: conversion
 //   instructions (F2I, I2F) run at the MUFU rate on sm_100 (16 per clock and SM, measured), these are plain FADDs.
 //   At an integer t either neighbour bin gives the same value (the interpolant is continuous), and
@@ -202,7 +210,7 @@ __device__ __forceinline__ void cb_point(const DevModel &m, const double *X, con
 __device__ __forceinline__ void bin_frac(float d2, float t0, float inv_delta, float tmax, float thmax, int &b, float &f)
 {
     float d;
-    asm("sqrt.approx.f32 %0, %1;" : "=f"(d) : "f"(d2));
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(d) : "f"(d2));
     float t = fmaf(d, inv_delta, t0);                        // (d - c0) / delta with t0 = -c0 / delta: one fma
     t = fminf(fmaxf(t, 0.0f), tmax);
     const float u = __fadd_rn(fminf(__fadd_rn(t, -0.5f), thmax), 12582912.0f);
@@ -268,7 +276,7 @@ template <bool RING>
 __device__ __forceinline__ float local_new_sum(const DevModel &m, const LocalTab &tb, const float4 *cb4, const float4 *cbn,
                                                int ilo, int split, int nI, int nJ, int glane, int gl)
 {
-    constexpr int U = 3;
+    constexpr int U = AMH_UL;
     const int nP = nI * nJ;
     float acc[U];
 #pragma unroll
@@ -286,7 +294,8 @@ __device__ __forceinline__ float local_new_sum(const DevModel &m, const LocalTab
             const float e = local_pair<RING>(m, tb, ci, pj);
             acc[u] += valid ? e : 0.0f;
             jj += gl;
-            while (jj >= nJ) { jj -= nJ; ++ii; }
+            if (jj >= nJ) { jj -= nJ; ++ii; }
+            while (jj >= nJ) { jj -= nJ; ++ii; }             // gl > nJ only at the chain ends
         }
     }
     float s = acc[0];
@@ -391,7 +400,7 @@ __device__ __forceinline__ double global_cols_sum(const DevModel &m, const float
             }
             // U rows per trip: all distances first, then all gathers, then the sums, so that a thread has U loads in
             // flight instead of stalling on each pair's row (the rows of near pairs come from L2, ~600 cycles away)
-            constexpr int U = 4;
+            constexpr int U = AMH_UG;
             float part = 0.0f;
 #pragma unroll
             for (int t = 0; t < kBlk / U; ++t) {
@@ -426,6 +435,27 @@ __device__ __forceinline__ double global_cols_sum(const DevModel &m, const float
     return acc;
 }
 
+// the column line of a global transition: sum of e' over (i, j), i = 0 .. cnt - 1, at the current positions
+__device__ __forceinline__ double global_col_sum(const DevModel &m, const float4 *cb4, int j, int cnt, int tid, int nthr)
+{
+    double acc = 0.0;
+    if (cnt <= 0) return acc;
+    const float4 cj = cb4[j];
+    for (int i = tid; i < cnt; i += nthr) {
+        const float4 ci = cb4[i];
+        const float dx = ci.x - cj.x, dy = ci.y - cj.y, dz = ci.z - cj.z;
+        const float d2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+        if (d2 < m.far2) {
+            int b;
+            float f;
+            bin_frac(d2, m.t0, m.inv_delta, m.tmax, m.thmax, b, f);
+            const float2 v = __ldg(m.Epk + (size_t)tri_row(i, j, m.L) * m.nb + b);
+            acc += (double)fmaf(f, v.y, v.x);
+        }
+    }
+    return acc;
+}
+
 // the row line of a global transition: sum of e' over (i, j), j = j0 .. j0 + cnt - 1, at the current positions
 __device__ __forceinline__ double global_row_sum(const DevModel &m, const float4 *cb4, int i, int j0, int cnt, int tid, int nthr)
 {
@@ -450,10 +480,26 @@ __device__ __forceinline__ double global_row_sum(const DevModel &m, const float4
 }
 
 // ---- exact-decision guard (R24) --------------------------------------------------------------
+// what the fp64 path needs of the model, passed BY VALUE: a reference to the kernel's DevModel parameter would force
+// that whole struct into local memory and turn every m.field of the hot loops into a local load
+struct ExactModel {
+    const float *P;
+    int L, nb, min_sep;
+    double c0_d, delta_d, eps_d, far2_d, inv_len_n_ca, inv_len_ca_c, cbA, cbB, cbC;
+};
+__device__ __forceinline__ ExactModel exact_model(const DevModel &m)
+{
+    ExactModel e;
+    e.P = m.P; e.L = m.L; e.nb = m.nb; e.min_sep = m.min_sep;
+    e.c0_d = m.c0_d; e.delta_d = m.delta_d; e.eps_d = m.eps_d; e.far2_d = m.far2_d;
+    e.inv_len_n_ca = m.inv_len_n_ca; e.inv_len_ca_c = m.inv_len_ca_c; e.cbA = m.cbA; e.cbB = m.cbB; e.cbC = m.cbC;
+    return e;
+}
+
 // dE of the proposal at variable k in fp64, every term from the fp64 atoms and from -log(p + eps) itself: this
 // thread's share of the sum over (i, j), ilo <= i < split <= j <= jhi, j - i >= min_sep, of e(new) - e(old).
 // Pairs beyond the last bin centre before and after contribute exactly 0 (R8's clamp) and are skipped.
-__device__ __noinline__ double exact_dE_partial(const DevModel &m, const double *X, const double *Y, const double *Z, int cb64,
+__device__ __noinline__ double exact_dE_partial(const ExactModel m, const double *X, const double *Y, const double *Z, int cb64,
                                                int k, double cd, double sd, int ilo, int jhi, int tid, int nthr)
 {
     const int L = m.L;
@@ -653,7 +699,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     if (slot >= nvalid) return;
 
     // ================= team: one chain =====================================================================
-    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L, a.cb64, a.nspec, a.wpts);
+    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L, a.cb64, a.nspec, a.wpts, W);
     constexpr bool cb64 = CB64;
     const int na = cb64 ? 4 : 3;                            // atoms per residue kept in fp64
     double *X = reinterpret_cast<double *>(cbase), *Y = X + na * L, *Z = Y + na * L;
@@ -686,7 +732,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     // exact-decision guard: the bound on the fp32 error of dE grows with the size of the coordinates (their fp32 rounding)
     double ext_scale = fmax(1.0, (double)team_extent(cb4, L, red, tid, nthreads, warp, nwarps, lane, bar_id) * (1.0 / 32.0));
     // local proposals are evaluated by groups of gl lanes, 32 / gl groups per warp
-    const int gshift = a.lanes_per_step == 8 ? 3 : (a.lanes_per_step == 16 ? 4 : 5);
+    const int gshift = a.lanes_per_step == 4 ? 2 : (a.lanes_per_step == 8 ? 3 : (a.lanes_per_step == 16 ? 4 : 5));
     const int gl = 1 << gshift, gpw = 32 >> gshift;
     const int grp = lane >> gshift, glane = lane & (gl - 1);
     const int nspec = a.nspec;
@@ -745,6 +791,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
             sigma_t = (t >= a.ramp_sigma - 1) ? a.sigma_end
                                               : a.sigma_start + (a.sigma_end - a.sigma_start) * ((double)t / (double)(a.ramp_sigma - 1));
         int seen_rel = -1;                                   // last column of this sweep the team has waited for
+        tb.c_ref = 0; tb.slot_c = slot_j0;                   // ring slot of the window centre, advanced with it
         int dead_rel = 0;                                    // columns < dead_rel of this sweep have been released (tid 0)
         const double guard = (gp ? a.guard_global : a.guard_local) * ext_scale * invT;
         double S_base = 0.0;                                 // S_old of step k - 1 for the current state (every thread holds it)
@@ -822,7 +869,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 if (k & 1) {                                  // the split moved: column c leaves, row c enters
                     const int c = k >> 1;
                     p_T = global_row_sum(m, cb4, c, c + m.min_sep, L - c - m.min_sep, tid, nthreads)
-                        - global_cols_sum(m, cb4, blk4, X, Y, Z, cb64, false, Rk, c, c, c, tid, nthreads);
+                        - global_col_sum(m, cb4, c, c - m.min_sep + 1, tid, nthreads);
                 }
                 team_sum2(p_new, p_T, red, warp, nwarps, lane, bar_id);
                 my_new = p_new; my_T = p_T;
@@ -842,9 +889,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                         if (++seen_slot == R) { seen_slot = 0; seen_par ^= 1u; }
                         mbar_wait(&full_bar[seen_slot], seen_par);
                     }
-                    tb.c_ref = c_now;
-                    tb.slot_c = slot_j0 + c_now;
-                    if (tb.slot_c >= R) tb.slot_c %= R;
+                    while (tb.c_ref < c_now) { ++tb.c_ref; if (++tb.slot_c == R) tb.slot_c = 0; }
                 }
                 const int r = gp ? warp : warp * gpw + grp;
                 const int gl_x = gp ? 32 : gl, glane_x = gp ? lane : glane;
@@ -869,7 +914,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                         }
                         if (kk & 1)
                             p_T = global_row_sum(m, cb4, c, c + m.min_sep, L - c - m.min_sep, lane, 32)
-                                - global_cols_sum(m, cb4, blk4, X, Y, Z, cb64, false, Rk, c, c, c, lane, 32);
+                                - global_col_sum(m, cb4, c, c - m.min_sep + 1, lane, 32);
                     }
                 } else {
                     // ---- a3/a4: in-window straddling pairs (Eq. 3b) ------------------------------------------------
@@ -933,7 +978,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 const int r0 = __ffs(m_go) - 1;
                 if (!((m_unc >> r0) & 1u)) { rsel = r0; break; }
                 const int kx = k + r0, bx = kx - batch_start, cx = kx >> 1;
-                const double dx = team_sum(exact_dE_partial(m, X, Y, Z, cb64 ? 1 : 0, kx, b_cd[bx], b_sd[bx],
+                const double dx = team_sum(exact_dE_partial(exact_model(m), X, Y, Z, cb64 ? 1 : 0, kx, b_cd[bx], b_sd[bx],
                                                             gp ? 0 : max(0, cx - w_eff), gp ? L - 1 : min(L - 1, cx + w_eff),
                                                             tid, nthreads), red, warp, nwarps, lane, bar_id);
                 const bool ax = b_lu[bx] <= -dx / T;
