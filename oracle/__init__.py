@@ -281,3 +281,142 @@ def run_pt(model: "Model", states, n_cycles: int, T, replicas: int, *, n_global=
         Tn, acc, _ = exchange(e, Tn, replicas, y, seed, chain_offset)
         n_try += len(acc); n_acc += sum(acc.values())
     return dict(states=s, T=Tn, energy=e, n_swap_tried=n_try, n_swap_accepted=n_acc)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# NEXT-2: config 3, trRosetta2-style energy on the 5-slot state (BASELINE.json:11; R25).  The arithmetic is
+# in amh_oracle.c ("NEXT-2" section); this only marshals.
+# ---------------------------------------------------------------------------------------------------------
+class _TR5Model(C.Structure):
+    _fields_ = [("L", C.c_int), ("nb_d", C.c_int), ("nb_o", C.c_int), ("nb_t", C.c_int), ("nb_p", C.c_int),
+                ("Ed", C.c_void_p), ("Eo", C.c_void_p), ("Et", C.c_void_p), ("Ep", C.c_void_p),
+                ("c0", C.c_double), ("delta", C.c_double), ("g", Geom)]
+
+
+def dihedral(a, b, c, d) -> float:
+    lib().amho_dihedral.restype = C.c_double
+    v = [np.ascontiguousarray(x, dtype=np.float64) for x in (a, b, c, d)]
+    return float(lib().amho_dihedral(*[_p(x) for x in v]))
+
+
+def angle(a, b, c) -> float:
+    lib().amho_angle.restype = C.c_double
+    v = [np.ascontiguousarray(x, dtype=np.float64) for x in (a, b, c)]
+    return float(lib().amho_angle(*[_p(x) for x in v]))
+
+
+def interp_periodic(row, x: float) -> float:
+    lib().amho_interp_periodic.restype = C.c_double
+    lib().amho_interp_periodic.argtypes = [C.c_void_p, C.c_int, C.c_double]
+    r = np.ascontiguousarray(row, dtype=np.float64)
+    return float(lib().amho_interp_periodic(_p(r), int(r.shape[0]), float(x)))
+
+
+def tr5_coords(s, geom: Geom | None = None):
+    """N, CA, C, CB (fp64 [L][3]) of one 5-slot state s (fp32 [5L]): R1 with omega_i = s[5i+2]."""
+    s = np.ascontiguousarray(s, dtype=np.float32)
+    L = s.shape[0] // 5
+    g = geom or default_geom()
+    out = [np.zeros((L, 3), dtype=np.float64) for _ in range(4)]
+    lib().amho_tr5_coords(C.byref(g), C.c_int(L), _p(s), *[_p(a) for a in out])
+    return tuple(out)
+
+
+def tr5_pair_geometry(s, geom: Geom | None = None):
+    """d, omega, theta, phi as [L][L] arrays of one state: entry [i][j] is the ORDERED pair (i, j) (diagonal 0)."""
+    N, CA, Cc, CB = tr5_coords(s, geom)
+    L = N.shape[0]
+    out = [np.zeros((L, L)) for _ in range(4)]
+    v = [C.c_double() for _ in range(4)]
+    f = lib().amho_tr5_pair_geometry
+    for i in range(L):
+        for j in range(L):
+            if i != j:
+                f(_p(N), _p(CA), _p(CB), C.c_int(i), C.c_int(j), *[C.byref(x) for x in v])
+                for q in range(4):
+                    out[q][i, j] = v[q].value
+    return tuple(out)
+
+
+class TR5Model:
+    """Config 3's energy: tables E = -log(p + eps) in fp64 for the distance, omega, theta and phi maps."""
+
+    def __init__(self, dist_p, edges, omega_p, theta_p, phi_p, geom: Geom | None = None):
+        self.geom = geom or default_geom()
+        self.L = int(dist_p.shape[0])
+        self.n = 5 * self.L
+        e = np.asarray(edges, dtype=np.float32).astype(np.float64)
+        self.nb = [int(a.shape[2]) for a in (dist_p, omega_p, theta_p, phi_p)]
+        self.delta = float((e[-1] - e[0]) / self.nb[0])
+        self.c0 = float(e[0] + 0.5 * self.delta)
+        self.E = []
+        for a in (dist_p, omega_p, theta_p, phi_p):
+            a = np.ascontiguousarray(a, dtype=np.float32)
+            assert a.shape[:2] == (self.L, self.L)
+            E = np.empty(a.shape, dtype=np.float64)
+            lib().amho_table(_p(a), C.c_longlong(a.size), C.c_double(self.geom.eps), _p(E))
+            self.E.append(E)
+        self._m = _TR5Model(self.L, *self.nb, *[x.ctypes.data for x in self.E], self.c0, self.delta, self.geom)
+        lib().amho_tr5_energy.restype = C.c_double
+        lib().amho_tr5_pair.restype = C.c_double
+
+    def energy(self, states, n_threads: int = 0) -> np.ndarray:
+        s = np.ascontiguousarray(states, dtype=np.float32).reshape(-1, self.n)
+        out = np.zeros(s.shape[0])
+        lib().amho_tr5_energy_batch(C.byref(self._m), _p(s), C.c_longlong(s.shape[0]), _p(out), C.c_int(n_threads))
+        return out
+
+    def energy_local(self, s, k: int, w: int) -> float:
+        s = np.ascontiguousarray(s, dtype=np.float32)
+        return float(lib().amho_tr5_energy(C.byref(self._m), _p(s), C.c_int(k), C.c_int(w), None))
+
+    def energy_atoms(self, N, CA, CB) -> float:
+        """V from given atoms (pins: rigid-motion invariance)."""
+        N, CA, CB = [np.ascontiguousarray(x, dtype=np.float64) for x in (N, CA, CB)]
+        v = 0.0
+        for i in range(self.L):
+            for j in range(i + self.geom.min_sep, self.L):
+                v += float(lib().amho_tr5_pair(C.byref(self._m), _p(N), _p(CA), _p(CB), C.c_int(i), C.c_int(j)))
+        return v
+
+    def _params(self, n_sweeps, kw):
+        d = dict(sweep_offset=0, n_global=1, n_local=10, window=12, global_first=True, t_start=1.0, t_end=1.0, ramp_sweeps=0,
+                 per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0, sigma_start=0.0, sigma_end=0.0, ramp_sigma=0, seed=1,
+                 chain_offset=0, trace_steps=0, n_threads=0)
+        bad = set(kw) - set(d)
+        if bad:
+            raise TypeError("unknown arguments %s" % sorted(bad))
+        d.update(kw)
+        pct = None if d["per_chain_T"] is None else np.ascontiguousarray(d["per_chain_T"], dtype=np.float32)
+        prm = _RunParams(n_sweeps, d["sweep_offset"], d["n_global"], d["n_local"], d["window"], int(d["global_first"]),
+                         d["t_start"], d["t_end"], d["ramp_sweeps"], None if pct is None else pct.ctypes.data,
+                         d["prop_mode"], d["grid"], d["sigma_start"], d["sigma_end"], d["ramp_sigma"], d["seed"],
+                         d["chain_offset"], -1, d["trace_steps"], d["n_threads"], 0)
+        return prm, pct, d
+
+    def run(self, states, n_sweeps, **kw):
+        s = np.array(states, dtype=np.float32, order="C").reshape(-1, self.n)
+        B = s.shape[0]
+        prm, keep, d = self._params(n_sweeps, kw)
+        ts = d["trace_steps"]
+        r = dict(energy=np.zeros(B), best_energy=np.zeros(B), best_state=np.zeros((B, self.n), np.float32),
+                 n_accept_local=np.zeros(B, np.int64), n_accept_global=np.zeros(B, np.int64), n_prop_local=None, n_prop_global=None,
+                 sweep_energy=None, trace_prop=np.zeros((B, ts), np.float32) if ts else None,
+                 trace_dE=np.zeros((B, ts)) if ts else None, trace_g=np.zeros((B, ts)) if ts else None,
+                 trace_acc=np.zeros((B, ts), np.uint8) if ts else None)
+        o = _Outputs(*[None if r[k] is None else r[k].ctypes.data for k, _ in _Outputs._fields_])
+        if lib().amho_tr5_run(C.byref(self._m), C.byref(prm), _p(s), C.c_longlong(B), C.byref(o)) != 0:
+            raise ValueError("amho_tr5_run: invalid argument")
+        r["states"] = s
+        return r
+
+    def follow(self, states, steps, forced_acc, **kw):
+        s = np.array(states, dtype=np.float32, order="C").reshape(-1, self.n)
+        B = s.shape[0]
+        fa = np.ascontiguousarray(forced_acc, dtype=np.uint8).reshape(B, steps)
+        prm, keep, d = self._params(0, kw)
+        prop = np.zeros((B, steps), np.float32); dE = np.zeros((B, steps)); g = np.zeros((B, steps)); acc = np.zeros((B, steps), np.uint8)
+        if lib().amho_tr5_follow(C.byref(self._m), C.byref(prm), _p(s), C.c_longlong(B), C.c_int(steps), _p(fa),
+                                 _p(prop), _p(dE), _p(g), _p(acc)) != 0:
+            raise ValueError("amho_tr5_follow: invalid argument")
+        return dict(states=s, prop=prop, dE=dE, g=g, acc=acc)

@@ -446,3 +446,255 @@ int amho_num_threads(void)
     return 1;
 #endif
 }
+
+/* =========================================================================================== */
+/* NEXT-2: config 3, trRosetta2-style energy on a 5-slot state (BASELINE.json:11; R25) */
+/* =========================================================================================== */
+/*
+ * The paper says only that "trRosetta2 follows a 5 angle parameterization" whose
+ * inter-residue geometry is "(phi, theta, omega)" and that "once the information is
+ * captured in the angle vector (s), the remaining procedure is unchanged".  Reading R25:
+ *   state   n = 5L, s[5i+0] = phi_i, s[5i+1] = psi_i, s[5i+2] = omega_i (the torsion of the peptide bond
+ *           C_i - N_{i+1}, a variable here instead of the constant 180 degrees of R1), s[5i+3], s[5i+4] = two
+ *           slots that move no backbone atom and no C-beta (their proposals have dE = 0: always accepted)
+ *   energy  V = sum over i < j, j - i >= min_sep of
+ *             e_d(|CB_i CB_j|)                                   37 bins over 2-20 A, R8's interpolation and clamp
+ *           + e_o(dihedral CA_i, CB_i, CB_j, CA_j)               24 bins over [-pi, pi), periodic, symmetric
+ *           + e_t[i][j](dihedral N_i, CA_i, CB_i, CB_j) + e_t[j][i](dihedral N_j, CA_j, CB_j, CB_i)   24 bins, periodic
+ *           + e_p[i][j](angle CA_i, CB_i, CB_j) + e_p[j][i](angle CA_j, CB_j, CB_i)                  12 bins over [0, pi], clamped
+ *           every e = -log(p + eps) interpolated linearly between bin centres (circularly for the periodic ones)
+ *   window  residue of variable k is floor(k/5); Eq. 3b and R12 unchanged
+ * Parity unpinned: the parameterisation itself and the orientation conventions (the paper fixes neither).
+ */
+typedef struct {
+    int L, nb_d, nb_o, nb_t, nb_p;
+    const double *Ed;      /* [L][L][nb_d]  i < j read */
+    const double *Eo;      /* [L][L][nb_o]  i < j read */
+    const double *Et;      /* [L][L][nb_t]  ordered: row (i, j) scores the dihedral seen from residue i */
+    const double *Ep;      /* [L][L][nb_p]  ordered */
+    double c0, delta;      /* distance bins: first centre, width */
+    amho_geom g;
+} amho_tr5_model;
+
+static double dot3(const double a[3], const double b[3]) { return a[0]*b[0] + a[1]*b[1] + a[2]*b[2]; }
+
+/* IUPAC dihedral a-b-c-d in (-pi, pi]: the angle between the projections of a-b and d-c on the plane normal to b-c */
+double amho_dihedral(const double a[3], const double b[3], const double c[3], const double d[3])
+{
+    double b0[3], b1[3], b2[3], v[3], w[3], x[3];
+    sub3(a, b, b0); sub3(c, b, b1); sub3(d, c, b2);
+    unit3(b1);
+    double p0 = dot3(b0, b1), p2 = dot3(b2, b1);
+    for (int q = 0; q < 3; ++q) { v[q] = b0[q] - p0 * b1[q]; w[q] = b2[q] - p2 * b1[q]; }
+    cross3(b1, v, x);
+    return atan2(dot3(x, w), dot3(v, w));
+}
+
+/* angle a-b-c at b in [0, pi] */
+double amho_angle(const double a[3], const double b[3], const double c[3])
+{
+    double u[3], v[3];
+    sub3(a, b, u); sub3(c, b, v);
+    double q = dot3(u, v) / sqrt(dot3(u, u) * dot3(v, v));
+    if (q > 1.0) q = 1.0;
+    if (q < -1.0) q = -1.0;
+    return acos(q);
+}
+
+/* periodic table over [-pi, pi): bin centres -pi + (b + 1/2) 2 pi / nb, circular linear interpolation */
+double amho_interp_periodic(const double *Erow, int nb, double x)
+{
+    const double two_pi = 6.283185307179586, delta = two_pi / nb;
+    double t = (x + 3.141592653589793) / delta - 0.5;
+    double fl = floor(t);
+    double f = t - fl;
+    long b = (long)fl % nb;
+    if (b < 0) b += nb;
+    long b1 = (b + 1) % nb;
+    return Erow[b] + f * (Erow[b1] - Erow[b]);
+}
+
+void amho_tr5_coords(const amho_geom *g, int L, const float *s, double *N, double *CA, double *C, double *CB)
+{
+    if (L <= 0) return;
+    N[0] = 0; N[1] = 0; N[2] = 0;
+    CA[0] = g->len_n_ca; CA[1] = 0; CA[2] = 0;
+    C[0] = CA[0] - g->len_ca_c * cos(g->ang_n_ca_c);
+    C[1] = g->len_ca_c * sin(g->ang_n_ca_c);
+    C[2] = 0;
+    for (int i = 0; i + 1 < L; ++i) {
+        double psi_i = (double)s[5 * i + 1], om_i = (double)s[5 * i + 2], phi_n = (double)s[5 * (i + 1)];
+        place(N  + 3*i, CA + 3*i, C  + 3*i,         g->len_c_n,  g->ang_ca_c_n, psi_i, N  + 3*(i+1));
+        place(CA + 3*i, C  + 3*i, N  + 3*(i+1),     g->len_n_ca, g->ang_c_n_ca, om_i,  CA + 3*(i+1));
+        place(C  + 3*i, N  + 3*(i+1), CA + 3*(i+1), g->len_ca_c, g->ang_n_ca_c, phi_n, C  + 3*(i+1));
+    }
+    for (int i = 0; i < L; ++i)
+        place(C + 3*i, N + 3*i, CA + 3*i, g->cb_len, g->cb_ang, g->cb_dih, CB + 3*i);
+}
+
+/* the four inter-residue coordinates of the ordered pair (i, j): d, omega (symmetric), theta_ij, phi_ij */
+void amho_tr5_pair_geometry(const double *N, const double *CA, const double *CB, int i, int j,
+                            double *d, double *omega, double *theta, double *phi)
+{
+    *d = dist3(CB + 3*i, CB + 3*j);
+    *omega = amho_dihedral(CA + 3*i, CB + 3*i, CB + 3*j, CA + 3*j);
+    *theta = amho_dihedral(N + 3*i, CA + 3*i, CB + 3*i, CB + 3*j);
+    *phi = amho_angle(CA + 3*i, CB + 3*i, CB + 3*j);
+}
+
+/* one unordered pair i < j: the six terms */
+double amho_tr5_pair(const amho_tr5_model *m, const double *N, const double *CA, const double *CB, int i, int j)
+{
+    const double pi = 3.141592653589793;
+    double d, om, th_ij, ph_ij, d2, om2, th_ji, ph_ji;
+    amho_tr5_pair_geometry(N, CA, CB, i, j, &d, &om, &th_ij, &ph_ij);
+    amho_tr5_pair_geometry(N, CA, CB, j, i, &d2, &om2, &th_ji, &ph_ji);
+    const size_t ij = (size_t)i * m->L + j, ji = (size_t)j * m->L + i;
+    const double dp = pi / m->nb_p;
+    double e = amho_pair(m->Ed + ij * m->nb_d, m->nb_d, m->c0, m->delta, d);
+    e += amho_interp_periodic(m->Eo + ij * m->nb_o, m->nb_o, om);
+    e += amho_interp_periodic(m->Et + ij * m->nb_t, m->nb_t, th_ij);
+    e += amho_interp_periodic(m->Et + ji * m->nb_t, m->nb_t, th_ji);
+    e += amho_pair(m->Ep + ij * m->nb_p, m->nb_p, 0.5 * dp, dp, ph_ij);
+    e += amho_pair(m->Ep + ji * m->nb_p, m->nb_p, 0.5 * dp, dp, ph_ji);
+    return e;
+}
+
+static double tr5_energy_range(const amho_tr5_model *m, const double *N, const double *CA, const double *CB, int lo, int hi)
+{
+    double v = 0.0;
+    for (int i = lo; i <= hi; ++i)
+        for (int j = i + m->g.min_sep; j <= hi; ++j)
+            v += amho_tr5_pair(m, N, CA, CB, i, j);
+    return v;
+}
+
+/* V (k < 0) or V_local(k, w) of one state; scratch = 12 L doubles */
+double amho_tr5_energy(const amho_tr5_model *m, const float *s, int k, int w, double *scratch)
+{
+    const int L = m->L;
+    double *own = scratch ? NULL : (double *)malloc(sizeof(double) * 12 * (size_t)L);
+    double *N = scratch ? scratch : own, *CA = N + 3 * L, *C = CA + 3 * L, *CB = C + 3 * L;
+    amho_tr5_coords(&m->g, L, s, N, CA, C, CB);
+    int lo = 0, hi = L - 1;
+    if (k >= 0) {
+        int c = k / 5;
+        lo = c - w < 0 ? 0 : c - w;
+        hi = c + w > L - 1 ? L - 1 : c + w;
+    }
+    double v = tr5_energy_range(m, N, CA, CB, lo, hi);
+    free(own);
+    return v;
+}
+
+void amho_tr5_energy_batch(const amho_tr5_model *m, const float *states, long long B, double *out, int n_threads)
+{
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+    long long n = 5LL * m->L;
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (long long b = 0; b < B; ++b) out[b] = amho_tr5_energy(m, states + b * n, -1, 0, NULL);
+}
+
+static double tr5_proposal_dE(const amho_tr5_model *m, const amho_run_params *p, int is_global, int k,
+                              float *s, float s_new, double *scratch)
+{
+    const int kk = is_global ? -1 : k;
+    double v0 = amho_tr5_energy(m, s, kk, p->window, scratch);
+    float keep = s[k];
+    s[k] = s_new;
+    double v1 = amho_tr5_energy(m, s, kk, p->window, scratch);
+    s[k] = keep;
+    return v1 - v0;
+}
+
+/* Alg. 1 on the 5-slot state: free-running (forced_acc == NULL) or follow mode (the first `steps` proposals
+ * of a run at sweep_offset, taking the decisions in forced_acc), exactly like amho_run / amho_follow */
+int amho_tr5_run(const amho_tr5_model *m, const amho_run_params *p, float *states, long long B, const amho_outputs *o)
+{
+    const int L = m->L, n = 5 * L;
+    if (L < 1 || B < 0 || p->n_global + p->n_local <= 0 || p->window < 0) return 1;
+#ifdef _OPENMP
+    if (p->n_threads > 0) omp_set_num_threads(p->n_threads);
+#endif
+    #pragma omp parallel
+    {
+        double *scratch = (double *)malloc(sizeof(double) * 12 * (size_t)L);
+        #pragma omp for schedule(dynamic, 1)
+        for (long long row = 0; row < B; ++row) {
+            float *s = states + row * n;
+            const uint64_t chain = (uint64_t)(p->chain_offset + row);
+            long long acc_l = 0, acc_g = 0, traced = 0;
+            double best = INFINITY, e_end = NAN;
+            for (long long t = p->sweep_offset; t < p->sweep_offset + p->n_sweeps; ++t) {
+                const int is_global = phase_is_global(p, t);
+                const double T = amho_temperature(p, t, row);
+                for (int k = 0; k < n; ++k) {
+                    const uint64_t step = (uint64_t)t * (uint64_t)n + (uint64_t)k;
+                    const float s_new = propose(p, chain, step, t, s[k]);
+                    const double dE = tr5_proposal_dE(m, p, is_global, k, s, s_new, scratch);
+                    const double lu = log(uniform01(p, chain, step));
+                    const int accept = lu <= -dE / T;
+                    if (traced < p->trace_steps) {
+                        size_t q = (size_t)row * p->trace_steps + traced;
+                        if (o->trace_prop) o->trace_prop[q] = s_new;
+                        if (o->trace_dE)   o->trace_dE[q] = dE;
+                        if (o->trace_g)    o->trace_g[q] = lu + dE / T;
+                        if (o->trace_acc)  o->trace_acc[q] = (unsigned char)accept;
+                        ++traced;
+                    }
+                    if (is_global) acc_g += accept; else acc_l += accept;
+                    if (accept) s[k] = s_new;
+                }
+                e_end = amho_tr5_energy(m, s, -1, 0, scratch);
+                if (e_end < best) {
+                    best = e_end;
+                    if (o->best_state) memcpy(o->best_state + row * n, s, sizeof(float) * n);
+                }
+            }
+            if (p->n_sweeps == 0) e_end = amho_tr5_energy(m, s, -1, 0, scratch);
+            if (o->energy) o->energy[row] = e_end;
+            if (o->best_energy) o->best_energy[row] = best;
+            if (o->n_accept_local)  o->n_accept_local[row]  = acc_l;
+            if (o->n_accept_global) o->n_accept_global[row] = acc_g;
+        }
+        free(scratch);
+    }
+    return 0;
+}
+
+int amho_tr5_follow(const amho_tr5_model *m, const amho_run_params *p, float *states, long long B, int steps,
+                    const unsigned char *forced_acc, float *own_prop, double *own_dE, double *own_g, unsigned char *own_acc)
+{
+    const int L = m->L, n = 5 * L;
+    if (L < 1 || p->n_global + p->n_local <= 0) return 1;
+#ifdef _OPENMP
+    if (p->n_threads > 0) omp_set_num_threads(p->n_threads);
+#endif
+    #pragma omp parallel
+    {
+        double *scratch = (double *)malloc(sizeof(double) * 12 * (size_t)L);
+        #pragma omp for schedule(dynamic, 1)
+        for (long long row = 0; row < B; ++row) {
+            float *s = states + row * n;
+            const uint64_t chain = (uint64_t)(p->chain_offset + row);
+            for (int q = 0; q < steps; ++q) {
+                const uint64_t step = (uint64_t)p->sweep_offset * (uint64_t)n + (uint64_t)q;
+                const long long t = (long long)(step / (uint64_t)n);
+                const int k = (int)(step % (uint64_t)n);
+                const int is_global = phase_is_global(p, t);
+                const double T = amho_temperature(p, t, row);
+                size_t z = (size_t)row * steps + q;
+                const float s_new = propose(p, chain, step, t, s[k]);
+                const double dE = tr5_proposal_dE(m, p, is_global, k, s, s_new, scratch);
+                const double lu = log(uniform01(p, chain, step));
+                own_prop[z] = s_new; own_dE[z] = dE; own_g[z] = lu + dE / T;
+                own_acc[z] = (unsigned char)(lu <= -dE / T);
+                if (forced_acc[z]) s[k] = s_new;
+            }
+        }
+        free(scratch);
+    }
+    return 0;
+}

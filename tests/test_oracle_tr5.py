@@ -1,0 +1,228 @@
+"""Pins P10-P15 of the NEXT-2 oracle: config 3's trRosetta2-style energy on the 5-slot state (BASELINE.json:11,
+PAPER.md:25, 125; R25).  The paper fixes neither the parameterisation nor the orientation conventions
+("parity unpinned" for those choices); what the mathematics fixes is pinned here: dihedral and angle against closed
+forms and against the NeRF construction that pin P1 ties to physical handedness, the circular interpolation, the
+symmetries of the terms, rigid-motion invariance, inert slots, window = global, and the Boltzmann law on L = 4.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy import stats
+
+import amh_inputs as gi
+
+
+def _dihedral_triple(a, b, c, d):
+    """the textbook triple-product form, typed independently of the oracle's projection form"""
+    b1, b2, b3 = b - a, c - b, d - c
+    return math.atan2(np.linalg.norm(b2) * np.dot(b1, np.cross(b2, b3)), np.dot(np.cross(b1, b2), np.cross(b2, b3)))
+
+
+@pytest.fixture(scope="module")
+def tr5(orc):
+    cache = {}
+
+    def make(L, cfg_seed=1003, min_sep=3):
+        key = (L, cfg_seed, min_sep)
+        if key not in cache:
+            ref = gi.reference_torsions_tr5(L, cfg_seed)
+            D, OM, TH, PH = orc.tr5_pair_geometry(ref)
+            maps = (gi.distogram_from_distances(D, n_bins=37, lo=2.0, hi=20.0),
+                    gi.periodic_map_from_values(OM, 24, -math.pi, math.pi, True),
+                    gi.periodic_map_from_values(TH, 24, -math.pi, math.pi, True),
+                    gi.periodic_map_from_values(PH, 12, 0.0, math.pi, False))
+            edges = gi.bin_edges(37, 2.0, 20.0)
+            cache[key] = (ref, maps, edges, orc.TR5Model(maps[0], edges, maps[1], maps[2], maps[3], orc.default_geom(min_sep=min_sep)))
+        return cache[key]
+    return make
+
+
+def test_dihedral_and_angle_closed_forms(orc):
+    # P10.  a on +x, axis b -> c along +z, d at azimuth t: IUPAC sign = sign of (b1 x b2) . b3
+    b, c = np.zeros(3), np.array([0.0, 0.0, 1.0])
+    a = np.array([1.0, 0.0, 0.0])
+    for t in np.linspace(-3.0, 3.0, 25):
+        d = np.array([math.cos(t), math.sin(t), 1.0 + 0.3])
+        got = orc.dihedral(a, b, c, d)
+        assert abs(got - _dihedral_triple(a, b, c, d)) < 1e-12
+        b1, b2, b3 = b - a, c - b, d - c
+        assert (got > 0) == (np.dot(np.cross(b1, b2), b3) > 0) or abs(got) < 1e-12
+        assert abs(abs(got) - abs(t)) < 1e-12                  # the azimuth itself, up to the sign convention
+    assert abs(orc.dihedral(a, b, c, np.array([1.0, 0.0, 1.0]))) < 1e-15                        # cis
+    assert abs(abs(orc.dihedral(a, b, c, np.array([-1.0, 0.0, 1.0]))) - math.pi) < 1e-15        # trans
+    # reversal keeps a dihedral, a mirror image flips it
+    rng = np.random.default_rng(1)
+    for _ in range(20):
+        p = rng.normal(size=(4, 3))
+        assert abs(orc.dihedral(*p) - orc.dihedral(*p[::-1])) < 1e-12
+        q = p * np.array([1.0, 1.0, -1.0])
+        assert abs(orc.dihedral(*p) + orc.dihedral(*q)) < 1e-12
+        assert abs(orc.dihedral(*p) - _dihedral_triple(*p)) < 1e-12
+    assert abs(orc.angle([1, 0, 0], [0, 0, 0], [0, 2, 0]) - math.pi / 2) < 1e-15
+    assert abs(orc.angle([1, 0, 0], [0, 0, 0], [0.5, math.sqrt(0.75), 0]) - math.pi / 3) < 1e-12
+    assert abs(orc.angle([1, 0, 0], [0, 0, 0], [-3, 0, 0]) - math.pi) < 1e-12
+    assert abs(orc.angle([1, 0, 0], [0, 0, 0], [5, 0, 0])) < 1e-7
+
+
+def test_nerf_with_variable_omega_round_trips(orc):
+    # the 5-slot NeRF: phi, psi AND omega measured back from the coordinates (the dihedral convention is the one pin P1
+    # ties to a right-handed helix); the two inert slots and phi_0, psi_{L-1}, omega_{L-1} move no atom
+    L = 12
+    s = gi.initial_states_tr5(1, L, 4)[0]
+    N, CA, Cc, CB = orc.tr5_coords(s)
+    for i in range(L - 1):
+        assert abs(orc.dihedral(N[i], CA[i], Cc[i], N[i + 1]) - s[5 * i + 1]) < 1e-6           # psi_i (fp32 input)
+        om = orc.dihedral(CA[i], Cc[i], N[i + 1], CA[i + 1])
+        assert min(abs(om - s[5 * i + 2]), abs(abs(om - s[5 * i + 2]) - 2 * math.pi)) < 1e-6   # omega_i
+        assert abs(orc.dihedral(Cc[i], N[i + 1], CA[i + 1], Cc[i + 1]) - s[5 * (i + 1)]) < 1e-6   # phi_{i+1}
+        assert abs(np.linalg.norm(N[i + 1] - Cc[i]) - 1.329) < 1e-12
+    base = np.concatenate(orc.tr5_coords(s))
+    for k in [0, 5 * (L - 1) + 1, 5 * (L - 1) + 2] + [5 * i + 3 for i in range(L)] + [5 * i + 4 for i in range(L)]:
+        t = s.copy(); t[k] = np.float32(0.123)
+        assert np.array_equal(np.concatenate(orc.tr5_coords(t)), base)
+    t = s.copy(); t[5 * 3 + 2] += np.float32(0.5)                  # an omega in the middle moves everything after it
+    assert np.abs(np.concatenate(orc.tr5_coords(t)) - base).max() > 0.1
+    # omega = pi in every residue reproduces the (phi, psi) chain of R1 (up to fp32(pi) - pi = 8.7e-8 rad per peptide bond)
+    s2 = gi.reference_torsions_tr5(L, 1003)
+    two = s2.reshape(L, 5)[:, :2].reshape(-1).copy()
+    for a, b in zip(orc.tr5_coords(s2), orc.coords(two)):
+        assert np.abs(a - b).max() < 2e-5
+
+
+def test_pair_geometry_symmetries_and_helix(orc):
+    L = 14
+    s = gi.initial_states_tr5(1, L, 6)[0]
+    D, OM, TH, PH = orc.tr5_pair_geometry(s)
+    off = ~np.eye(L, dtype=bool)
+    assert np.abs(D - D.T).max() < 1e-12 and np.abs(OM - OM.T)[off].max() < 1e-9       # d and omega are symmetric
+    assert np.abs(TH - TH.T)[off].max() > 0.1 and np.abs(PH - PH.T)[off].max() > 0.1     # theta and phi are not
+    assert np.all((PH[off] >= 0) & (PH[off] <= math.pi)) and np.all(np.abs(OM) <= math.pi) and np.all(np.abs(TH) <= math.pi)
+    # an ideal helix is invariant under its screw: the geometry of (i, i + k) depends on k only
+    h = np.zeros((L, 5), np.float32)
+    h[:, 0] = math.radians(-57.8); h[:, 1] = math.radians(-47.0); h[:, 2] = math.pi
+    Dh, OMh, THh, PHh = orc.tr5_pair_geometry(h.reshape(-1))
+    for k in (3, 4, 7):
+        for A in (Dh, OMh, THh, PHh):
+            up = np.array([A[i, i + k] for i in range(1, L - k - 1)]); dn = np.array([A[i + k, i] for i in range(1, L - k - 1)])
+            assert np.ptp(up) < 1e-9 and np.ptp(dn) < 1e-9
+
+
+def test_interpolation_periodic_and_clamped(orc):
+    # P13: value at a bin centre = the table entry; circular: the seam is continuous and the midpoint between the last
+    # and the first centre is their average; linear in between
+    rng = np.random.default_rng(3)
+    nb = 24
+    row = rng.normal(size=nb)
+    delta = 2 * math.pi / nb
+    cen = -math.pi + (np.arange(nb) + 0.5) * delta
+    for b in range(nb):
+        assert abs(orc.interp_periodic(row, cen[b]) - row[b]) < 1e-12
+        mid = orc.interp_periodic(row, cen[b] + 0.25 * delta)
+        assert abs(mid - (0.75 * row[b] + 0.25 * row[(b + 1) % nb])) < 1e-12
+    assert abs(orc.interp_periodic(row, -math.pi) - 0.5 * (row[0] + row[-1])) < 1e-12
+    assert abs(orc.interp_periodic(row, math.pi - 1e-13) - 0.5 * (row[0] + row[-1])) < 1e-9
+    assert abs(orc.interp_periodic(row, -math.pi + 0.1 * delta) - (0.4 * row[-1] + 0.6 * row[0])) < 1e-12
+
+
+def test_energy_invariances_and_reference(orc, tr5):
+    L = 24
+    ref, maps, edges, m = tr5(L)
+    s = gi.initial_states_tr5(4, L, 2)
+    V = m.energy(s)
+    # P12: rigid motion
+    rng = np.random.default_rng(0)
+    Q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+    if np.linalg.det(Q) < 0:
+        Q[:, 0] = -Q[:, 0]
+    t = rng.normal(size=3) * 30
+    for b in range(2):
+        N, CA, Cc, CB = orc.tr5_coords(s[b])
+        assert abs(m.energy_atoms(N, CA, CB) - V[b]) < 1e-9 * abs(V[b])
+        assert abs(m.energy_atoms(N @ Q.T + t, CA @ Q.T + t, CB @ Q.T + t) - V[b]) < 1e-9 * abs(V[b])
+        # a mirror image is NOT the same structure for the dihedral terms (chirality is scored)
+        assert abs(m.energy_atoms(N * [1, 1, -1], CA * [1, 1, -1], CB * [1, 1, -1]) - V[b]) > 1.0
+    # P14: the reference scores at the lower bound of its own maps, far below random states
+    npairs = (L - 3) * (L - 2) // 2
+    Eall = [-np.log(x.astype(np.float64) + 1e-8) for x in maps]
+    iu = [(i, j) for i in range(L) for j in range(i + 3, L)]
+    bound = sum(Eall[0][i, j].min() + Eall[1][i, j].min() + Eall[2][i, j].min() + Eall[2][j, i].min()
+                + Eall[3][i, j].min() + Eall[3][j, i].min() for i, j in iu)
+    vref = float(m.energy(ref[None])[0])
+    assert bound - 1e-9 <= vref <= bound + 0.08 * 6 * npairs
+    assert V.min() > vref + 1.0 * npairs
+    # window wider than the chain = global, and V_local against a brute-force masked sum
+    assert abs(m.energy_local(s[0], 37, L) - V[0]) < 1e-9 * abs(V[0])
+    N, CA, Cc, CB = orc.tr5_coords(s[1])
+    for k, w in ((0, 4), (5 * 9 + 2, 5), (5 * (L - 1) + 4, 3)):
+        c = k // 5; lo, hi = max(0, c - w), min(L - 1, c + w)
+        sub = orc.TR5Model(*[x[lo:hi + 1, lo:hi + 1] for x in (maps[0],)], edges, *[x[lo:hi + 1, lo:hi + 1] for x in maps[1:]])
+        want = sub.energy_atoms(N[lo:hi + 1], CA[lo:hi + 1], CB[lo:hi + 1])
+        assert abs(m.energy_local(s[1], k, w) - want) < 1e-9 * max(1.0, abs(want))
+    # min_sep
+    m1 = tr5(L, min_sep=5)[3]
+    assert m1.energy(s[:1])[0] < V[0]
+
+
+def test_run_schedule_inert_slots_and_follow(orc, tr5):
+    L = 10
+    ref, maps, edges, m = tr5(L)
+    s0 = gi.initial_states_tr5(6, L, 3)
+    kw = dict(n_global=1, n_local=2, window=3, seed=7, chain_offset=2)
+    n = 5 * L
+    r = m.run(s0, 6, trace_steps=6 * n, **kw)
+    acc, dE = r["trace_acc"], r["trace_dE"]
+    k = np.arange(6 * n) % n
+    inert = (k % 5 >= 3) | (k == 0) | (k == n - 4) | (k == n - 3)      # two inert slots, phi_0, psi_{L-1}, omega_{L-1}
+    assert np.all(dE[:, inert] == 0.0) and np.all(acc[:, inert] == 1)
+    assert np.abs(dE[:, ~inert]).min() > 0.0 and 0 < acc[:, ~inert].mean() < 1
+    assert np.array_equal(acc.astype(bool), r["trace_g"] <= 0.0)
+    # reported energies are the energies of the returned states; determinism; split runs compose
+    assert np.allclose(r["energy"], m.energy(r["states"]), rtol=1e-12)
+    assert np.allclose(r["best_energy"], m.energy(r["best_state"]), rtol=1e-12)
+    r2 = m.run(s0, 6, **kw)
+    assert np.array_equal(r2["states"], r["states"])
+    a = m.run(s0, 2, **kw); b = m.run(a["states"], 4, sweep_offset=2, **kw)
+    assert np.array_equal(b["states"], r["states"])
+    # follow mode reproduces the free run when it is fed its own decisions
+    f = m.follow(s0, 6 * n, acc, **kw)
+    assert np.array_equal(f["states"], r["states"]) and np.array_equal(f["acc"], acc) and np.array_equal(f["dE"], dE)
+
+
+def test_global_mh_samples_the_boltzmann_law_tr5_L4(orc, tr5):
+    # P15 (Eq. 1a-1c on the 5-slot state): L = 4, min_sep 3 -> one pair (0, 3) with all six terms; the nine torsions that
+    # move an atom (phi_1..3, psi_0..2, omega_0..2) on a 3-point grid give 3^9 = 19,683 states, enumerated.
+    # T = 3: at T = 1 the six-term energy (range 7.6 .. 36) splits the 3-point grid into basins that single flips do not
+    # connect within any run of practical length, and the test would measure the start distribution instead of the kernel
+    L, G, n, T = 4, 3, 20, 3.0
+    ref, maps, edges, m = tr5(L)
+    eff = [1, 2, 5, 6, 7, 10, 11, 12, 15]
+    idx = np.stack(np.meshgrid(*[np.arange(G)] * 9, indexing="ij"), -1).reshape(-1, 9)
+    gv = lambda mm: np.float32((2 * mm - G) / np.float32(G)) * np.float32(math.pi)
+    states = np.zeros((len(idx), n), np.float32)
+    for q, v in enumerate(eff):
+        states[:, v] = gv(idx[:, q])
+    V = m.energy(states)
+    assert V.max() - V.min() > 3.0
+    w = np.exp(-(V - V.min()) / T)
+    prob = w / w.sum()
+    B = 98304
+    start = gi.grid_states(B, n, G, seed=13)
+    r = m.run(start, 100, n_global=1, n_local=0, window=0, prop_mode=orc.PROP_GRID, grid=G, seed=9, t_start=T, t_end=T)
+    s = r["states"]
+    cell = np.zeros(B, np.int64)
+    for v in eff:
+        mm = np.rint((s[:, v].astype(np.float64) / math.pi * G + G) / 2).astype(np.int64)
+        assert np.all((mm >= 0) & (mm < G))
+        cell = cell * G + mm
+    counts = np.bincount(cell, minlength=G ** 9).astype(float)
+    expect = B * prob
+    small = expect < 5.0
+    c = np.concatenate([counts[~small], [counts[small].sum()]]); e = np.concatenate([expect[~small], [expect[small].sum()]])
+    pval = float(stats.chi2.sf(((c - e) ** 2 / e).sum(), len(e) - 1))
+    assert len(e) > 500 and pval > 0.01, (pval, len(e))
+    # the inert slots stay uniform on the grid
+    for v in (3, 4, 8, 0):
+        mm = np.rint((s[:, v].astype(np.float64) / math.pi * G + G) / 2).astype(np.int64)
+        cnt = np.bincount(mm, minlength=G)
+        assert stats.chisquare(cnt).pvalue > 0.001
