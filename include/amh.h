@@ -48,7 +48,8 @@ typedef enum {
 
 typedef enum {
     AMH_PARAM_PHI_PSI = 0,     /* 2 variables per residue (the paper's AlphaFold1 mapping) */
-    AMH_PARAM_TR5 = 1          /* 5 variables per residue (trRosetta2): not built, AMH_ERR_UNSUPPORTED */
+    AMH_PARAM_TR5 = 1          /* 5 variables per residue (trRosetta2; config 3): contexts of this kind are
+                                  built by amh_create_tr5(), which also takes the orientation maps */
 } amh_param;
 
 /* Geometry, energy and numerics options (the MODEL; nothing about the launch).  amh_default_options() fills the
@@ -148,7 +149,7 @@ amh_status amh_set_launch_options(amh_ctx *ctx, const amh_launch_options *opt);
 /* Build a context: validate, compute E = -log(p + eps) (Eq. 3a) into device memory.
  *   out         host; receives the context
  *   n_res       L >= 1 (L < min_sep + 1 is valid: no pairs, energy 0)
- *   param       AMH_PARAM_PHI_PSI
+ *   param       AMH_PARAM_PHI_PSI (AMH_PARAM_TR5: INVALID_ARG, use amh_create_tr5)
  *   distogram   HOST or DEVICE float [L][L][n_bins] row-major, p_ij(b) >= 0 finite; only i < j is read.
  *               Copied: the caller may free it after the call.
  *   bin_edges   HOST float [n_bins + 1], increasing, evenly spaced to 1e-5 relative (else UNSUPPORTED)
@@ -157,6 +158,37 @@ amh_status amh_set_launch_options(amh_ctx *ctx, const amh_launch_options *opt);
  * Synchronises the stream. */
 amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *distogram,
                       const float *bin_edges, int n_bins, const amh_options *opt, void *cuda_stream);
+
+/* Config 3 (NEXT-2; BASELINE.json:11; PAPER.md:25 "trRosetta2 follows a 5 angle parameterization", :125 "(phi, theta,
+ * omega)"; reading R25 of DESIGN.md - the paper fixes neither the parameterisation nor the orientation conventions).
+ *   state   n = 5 L variables per chain: s[5i+0] = phi_i, s[5i+1] = psi_i, s[5i+2] = omega_i (torsion of the peptide bond
+ *           C_i - N_{i+1}; geometry as R1 with this omega instead of the constant), s[5i+3], s[5i+4] = two slots that move
+ *           no backbone atom and no C-beta (their proposals have dE = 0 and are always accepted); the residue of variable
+ *           k is floor(k / 5)
+ *   energy  V = sum over i < j, j - i >= min_sep of
+ *               e_d(|CB_i CB_j|)                                 distogram, n_bins over the given edges (R8)
+ *             + e_o(dihedral CA_i, CB_i, CB_j, CA_j)             omega map, nb_omega bins over [-pi, pi), periodic
+ *             + e_t[i][j](dihedral N_i, CA_i, CB_i, CB_j) + e_t[j][i](dihedral N_j, CA_j, CB_j, CB_i)     theta map, periodic
+ *             + e_p[i][j](angle CA_i, CB_i, CB_j) + e_p[j][i](angle CA_j, CB_j, CB_i)    phi map, nb_phi bins over [0, pi]
+ *           every e = -log(p + eps) interpolated linearly between bin centres: clamped beyond the end centres (distance,
+ *           phi), circularly (omega, theta); IUPAC dihedrals in (-pi, pi]
+ *   maps    HOST or DEVICE float, row-major: omega [L][L][nb_omega] (only i < j is read), theta [L][L][nb_theta] and
+ *           phi [L][L][nb_phi] (entry [i][j] scores the geometry seen from residue i: both orders are read)
+ * amh_energy, amh_energy_local, amh_coords, amh_run and amh_run_host work on such a context with n = 5 L; the arithmetic
+ * is fp64 throughout (no decision guard is needed: trace_acc carries bit 1 on every step); amh_exchange / amh_run_pt too. */
+typedef struct {
+    const float *omega, *theta, *phi;
+    int nb_omega, nb_theta, nb_phi;
+} amh_orientation_maps;
+
+amh_status amh_create_tr5(amh_ctx **out, int n_res, const float *distogram, const float *bin_edges, int n_bins,
+                          const amh_orientation_maps *maps, const amh_options *opt, void *cuda_stream);
+
+/* The inter-residue geometry of config 3 for a batch of 5-slot states (the reference structure's values, from which
+ * synthetic orientation maps are drawn): DEVICE double [B][L][L] each, entry [i][j] = the ORDERED pair (i, j) - distance
+ * |CB_i CB_j|, omega_ij, theta_ij, phi_ij (0 on the diagonal); any output may be NULL.  TR5 contexts only. */
+amh_status amh_pair_geometry(amh_ctx *ctx, const float *states, long long B, double *d_out, double *omega_out,
+                             double *theta_out, double *phi_out, void *cuda_stream);
 
 /* Free the context and everything it owns (synchronises the device). NULL is allowed. */
 amh_status amh_destroy(amh_ctx *ctx);

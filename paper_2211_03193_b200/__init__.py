@@ -24,7 +24,7 @@ PROP_UNIFORM, PROP_GRID, PROP_GAUSSIAN = 0, 1, 2
 
 # every symbol include/amh.h declares
 EXPORTS = ["amh_default_options", "amh_default_launch_options", "amh_set_launch_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
-           "amh_run", "amh_run_host", "amh_run_pt", "amh_exchange", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
+           "amh_create_tr5", "amh_pair_geometry", "amh_run", "amh_run_host", "amh_run_pt", "amh_exchange", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
            "amh_last_error", "amh_version"]
 
 
@@ -63,6 +63,11 @@ class Options:
             if k in dict(st._fields_):
                 return setattr(st, k, v)
         raise AttributeError(k)
+
+
+class _OrientationMaps(C.Structure):       # amh_orientation_maps
+    _fields_ = [("omega", C.c_void_p), ("theta", C.c_void_p), ("phi", C.c_void_p),
+                ("nb_omega", C.c_int), ("nb_theta", C.c_int), ("nb_phi", C.c_int)]
 
 
 class _Schedule(C.Structure):
@@ -106,6 +111,8 @@ def lib():
         L.amh_version.restype = C.c_char_p
         L.amh_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int,
                                  C.c_void_p, C.c_void_p]
+        L.amh_create_tr5.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.amh_pair_geometry.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.amh_destroy.argtypes = [C.c_void_p]
         L.amh_energy.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p]
         L.amh_energy_host.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p]
@@ -179,7 +186,8 @@ def philox4x32_10(ctr, key):
 class AMH:
     """amh_ctx: energy table on the device + geometry constants (amh_create / amh_destroy)."""
 
-    def __init__(self, distogram, bin_edges, options: Options | None = None, stream=None):
+    def __init__(self, distogram, bin_edges, options: Options | None = None, stream=None, orientation=None):
+        """orientation = (omega, theta, phi) maps, each [L][L][bins]: amh_create_tr5 (config 3, n = 5 L variables per chain)."""
         torch = _torch()
         self._h = C.c_void_p()
         if isinstance(distogram, torch.Tensor):
@@ -194,10 +202,21 @@ class AMH:
         if e.shape != (shape[2] + 1,):
             raise ValueError("bin_edges must be [n_bins + 1]")
         self.L, self.n_bins = int(shape[0]), int(shape[2])
-        self.n = 2 * self.L
         self.options = options
-        _check(lib().amh_create(C.byref(self._h), self.L, 0, dptr, e.ctypes.data, self.n_bins,
-                                C.byref(options.model) if options is not None else None, _stream_ptr(stream)))
+        optp = C.byref(options.model) if options is not None else None
+        if orientation is None:
+            self.n = 2 * self.L
+            _check(lib().amh_create(C.byref(self._h), self.L, 0, dptr, e.ctypes.data, self.n_bins, optp, _stream_ptr(stream)))
+        else:
+            self.n = 5 * self.L
+            keep = [np.ascontiguousarray(a, dtype=np.float32) for a in orientation]
+            for a in keep:
+                if a.ndim != 3 or a.shape[:2] != (self.L, self.L):
+                    raise ValueError("orientation maps must be [L][L][bins]")
+            om = _OrientationMaps(keep[0].ctypes.data, keep[1].ctypes.data, keep[2].ctypes.data,
+                                  keep[0].shape[2], keep[1].shape[2], keep[2].shape[2])
+            _check(lib().amh_create_tr5(C.byref(self._h), self.L, dptr, e.ctypes.data, self.n_bins, C.byref(om), optp,
+                                        _stream_ptr(stream)))
         if options is not None:
             try:
                 _check(lib().amh_set_launch_options(self._h, C.byref(options.launch)))
@@ -248,6 +267,15 @@ class AMH:
         _check(lib().amh_coords(self._h, s.data_ptr(), B, cb.data_ptr(), at.data_ptr() if atoms else None,
                                 _stream_ptr(stream)))
         return (cb, at) if atoms else cb
+
+    def pair_geometry(self, states, stream=None):
+        """amh_pair_geometry (config 3): d, omega, theta, phi as fp64 [B][L][L] device tensors."""
+        torch = _torch()
+        s = _dev(states, torch.float32, "states").reshape(-1, self.n)
+        B = s.shape[0]
+        out = [torch.empty((B, self.L, self.L), dtype=torch.float64, device="cuda") for _ in range(4)]
+        _check(lib().amh_pair_geometry(self._h, s.data_ptr(), B, *[o.data_ptr() for o in out], _stream_ptr(stream)))
+        return tuple(out)
 
     def launch_info(self, B: int, window: int = 0) -> dict:
         v = [C.c_int() for _ in range(4)]

@@ -10,6 +10,7 @@
 #include "../../include/amh.h"
 #include "amh_kernels.cuh"
 #include "amh_sweep.cuh"
+#include "amh_tr5.cuh"
 
 namespace {
 
@@ -55,6 +56,9 @@ struct amh_ctx {
     float *Ebd = nullptr;        // the band j - i <= band_dmax of the same E', column-major, rows padded to row_stride floats (TMA source)
     int band_dmax = 0;
     float *P = nullptr;          // the probabilities themselves (fp64 path of the exact-decision guard)
+    int param = AMH_PARAM_PHI_PSI;
+    amh::Tr5Model tm;            // config 3 (AMH_PARAM_TR5): fp64 tables
+    double *tE[4] = {nullptr, nullptr, nullptr, nullptr};
     int device = 0, n_sm = 0, max_smem = 0;
     // staging for the *_host calls (grow-only)
     void *stage = nullptr;
@@ -128,7 +132,7 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
 {
     if (!out) return fail(AMH_ERR_INVALID_ARG, "amh_create: out is NULL");
     *out = nullptr;
-    if (param == AMH_PARAM_TR5) return fail(AMH_ERR_UNSUPPORTED, "amh_create: AMH_PARAM_TR5 (config 3) is not built");
+    if (param == AMH_PARAM_TR5) return fail(AMH_ERR_INVALID_ARG, "amh_create: AMH_PARAM_TR5 contexts are built by amh_create_tr5 (it takes the orientation maps)");
     if (param != AMH_PARAM_PHI_PSI) return fail(AMH_ERR_INVALID_ARG, "amh_create: unknown parameterisation %d", (int)param);
     if (n_res < 1) return fail(AMH_ERR_INVALID_ARG, "amh_create: n_res = %d < 1", n_res);
     if (n_bins < 2) return fail(AMH_ERR_INVALID_ARG, "amh_create: n_bins = %d < 2", n_bins);
@@ -286,6 +290,136 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     return AMH_OK;
 }
 
+amh_status amh_create_tr5(amh_ctx **out, int n_res, const float *distogram, const float *bin_edges, int n_bins,
+                          const amh_orientation_maps *maps, const amh_options *opt, void *cuda_stream)
+{
+    if (!out) return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: out is NULL");
+    *out = nullptr;
+    if (n_res < 1) return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: n_res = %d < 1", n_res);
+    if (n_bins < 2) return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: n_bins = %d < 2", n_bins);
+    if (!distogram || !bin_edges || !maps || !maps->omega || !maps->theta || !maps->phi)
+        return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: distogram / bin_edges / maps is NULL");
+    if (maps->nb_omega < 2 || maps->nb_theta < 2 || maps->nb_phi < 2)
+        return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: every orientation map needs at least 2 bins");
+    amh_options o;
+    amh_default_options(&o);
+    if (opt) o = *opt;
+    if (o.min_sep < 1) return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: min_sep = %d < 1", o.min_sep);
+    if (!(o.eps >= 0.0)) return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: eps < 0");
+    for (int b = 0; b <= n_bins; ++b)
+        if (!std::isfinite(bin_edges[b])) return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: bin edge %d is not finite", b);
+    const double e0 = bin_edges[0], e1 = bin_edges[n_bins];
+    const double delta = (e1 - e0) / n_bins;
+    if (!(delta > 0.0)) return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: bin edges do not increase");
+    for (int b = 0; b < n_bins; ++b) {
+        const double w = (double)bin_edges[b + 1] - (double)bin_edges[b];
+        if (!(w > 0.0)) return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: bin edges do not increase at %d", b);
+        if (std::fabs(w - delta) > 1e-5 * delta)
+            return fail(AMH_ERR_UNSUPPORTED, "amh_create_tr5: bins are not evenly spaced (bin %d: %g vs %g)", b, w, delta);
+    }
+    amh_ctx *c = new (std::nothrow) amh_ctx;
+    if (!c) return fail(AMH_ERR_OOM, "amh_create_tr5: host allocation failed");
+    c->opt = o;
+    c->param = AMH_PARAM_TR5;
+    amh_default_launch_options(&c->lopt);
+    std::memset(&c->m, 0, sizeof c->m);
+    cudaError_t e = cudaGetDevice(&c->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device);
+    if (e != cudaSuccess) { delete c; return fail(AMH_ERR_CUDA, "amh_create_tr5: no usable CUDA device: %s", cudaGetErrorString(e)); }
+    if (amh::tr5_smem_bytes(n_res, true) > (size_t)c->max_smem - 1024) {
+        delete c;
+        return fail(AMH_ERR_UNSUPPORTED, "amh_create_tr5: L = %d needs %zu B of shared memory per chain, device allows %d", n_res,
+                    amh::tr5_smem_bytes(n_res, true), c->max_smem);
+    }
+    c->m.L = n_res; c->m.n = 5 * n_res; c->m.nb = n_bins; c->m.min_sep = o.min_sep;
+    amh::Tr5Model &t = c->tm;
+    t.L = n_res; t.n = 5 * n_res; t.nb_d = n_bins; t.nb_o = maps->nb_omega; t.nb_t = maps->nb_theta; t.nb_p = maps->nb_phi;
+    t.min_sep = o.min_sep;
+    t.c0 = e0 + 0.5 * delta; t.delta = delta;
+    t.A = mplus(o.ang_n_ca_c, 0.0, o.len_ca_c);
+    t.c2 = std::cos(o.ang_ca_c_n); t.s2 = std::sin(o.ang_ca_c_n); t.l3 = o.len_c_n;
+    t.c3 = std::cos(o.ang_c_n_ca); t.s3 = std::sin(o.ang_c_n_ca); t.l1 = o.len_n_ca;
+    t.loc[0][0] = -o.len_n_ca; t.loc[0][1] = 0.0; t.loc[0][2] = 0.0;
+    t.loc[1][0] = 0.0; t.loc[1][1] = 0.0; t.loc[1][2] = 0.0;
+    t.loc[2][0] = -o.len_ca_c * std::cos(o.ang_n_ca_c); t.loc[2][1] = o.len_ca_c * std::sin(o.ang_n_ca_c); t.loc[2][2] = 0.0;
+    t.loc[3][0] = -o.cb_len * std::cos(o.cb_ang);
+    t.loc[3][1] = o.cb_len * std::sin(o.cb_ang) * std::cos(o.cb_dih);
+    t.loc[3][2] = o.cb_len * std::sin(o.cb_ang) * std::sin(o.cb_dih);
+    t.h0x = o.len_n_ca;
+    t.inv_len_n_ca = 1.0 / o.len_n_ca; t.inv_len_ca_c = 1.0 / o.len_ca_c; t.inv_len_c_n = 1.0 / o.len_c_n;
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int *bad_dev = nullptr;
+    float *p_dev = nullptr;
+    auto cleanup = [&]() {
+        if (bad_dev) cudaFree(bad_dev);
+        if (p_dev) cudaFree(p_dev);
+        for (double *q : c->tE) if (q) cudaFree(q);
+        delete c;
+    };
+#define AMH_CUDA_T(call)                                                                           \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            cleanup();                                                                             \
+            return fail(e_ == cudaErrorMemoryAllocation ? AMH_ERR_OOM : AMH_ERR_CUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                   \
+        }                                                                                          \
+    } while (0)
+    AMH_CUDA_T(cudaMalloc(&bad_dev, sizeof(int)));
+    AMH_CUDA_T(cudaMemsetAsync(bad_dev, 0, sizeof(int), st));
+    const float *src[4] = {distogram, maps->omega, maps->theta, maps->phi};
+    const int nbs[4] = {n_bins, maps->nb_omega, maps->nb_theta, maps->nb_phi};
+    size_t max_count = 0;
+    for (int q = 0; q < 4; ++q) max_count = std::max(max_count, (size_t)n_res * n_res * nbs[q]);
+    for (int q = 0; q < 4; ++q) {
+        const size_t count = (size_t)n_res * n_res * nbs[q];
+        AMH_CUDA_T(cudaMalloc(&c->tE[q], sizeof(double) * count));
+        cudaPointerAttributes at;
+        const bool on_device = (cudaPointerGetAttributes(&at, src[q]) == cudaSuccess) &&
+                               (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged);
+        cudaGetLastError();
+        const float *ps = src[q];
+        if (!on_device) {
+            if (!p_dev) AMH_CUDA_T(cudaMalloc(&p_dev, sizeof(float) * max_count));
+            AMH_CUDA_T(cudaMemcpyAsync(p_dev, src[q], sizeof(float) * count, cudaMemcpyHostToDevice, st));
+            ps = p_dev;
+        }
+        const int blocks = (int)std::min<size_t>((count + 255) / 256, (size_t)c->n_sm * 16);
+        amh::tr5_table_kernel<<<blocks, 256, 0, st>>>(ps, c->tE[q], (long long)count, o.eps, bad_dev);
+        AMH_CUDA_T(cudaGetLastError());
+    }
+    int bad = 0;
+    AMH_CUDA_T(cudaMemcpyAsync(&bad, bad_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
+    AMH_CUDA_T(cudaStreamSynchronize(st));
+    if (bad) { cleanup(); return fail(AMH_ERR_INVALID_ARG, "amh_create_tr5: a map holds a negative, NaN or infinite value"); }
+    cudaFree(bad_dev); bad_dev = nullptr;
+    if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
+    t.Ed = c->tE[0]; t.Eo = c->tE[1]; t.Et = c->tE[2]; t.Ep = c->tE[3];
+    AMH_CUDA_T(cudaFuncSetAttribute(amh::tr5_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem - 1024));   // it also has a few static words
+    AMH_CUDA_T(cudaFuncSetAttribute(amh::tr5_energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+    AMH_CUDA_T(cudaFuncSetAttribute(amh::tr5_geometry_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
+#undef AMH_CUDA_T
+    *out = c;
+    return AMH_OK;
+}
+
+amh_status amh_pair_geometry(amh_ctx *c, const float *states, long long B, double *d_out, double *omega_out,
+                             double *theta_out, double *phi_out, void *cuda_stream)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_pair_geometry: ctx is NULL");
+    if (c->param != AMH_PARAM_TR5) return fail(AMH_ERR_INVALID_ARG, "amh_pair_geometry: needs an AMH_PARAM_TR5 context");
+    if (B < 0) return fail(AMH_ERR_INVALID_ARG, "amh_pair_geometry: B = %lld < 0", B);
+    if (B == 0) return AMH_OK;
+    if (!states) return fail(AMH_ERR_INVALID_ARG, "amh_pair_geometry: states is NULL");
+    const int blocks = (int)std::min<long long>(B, (long long)c->n_sm * 16);
+    amh::tr5_geometry_kernel<<<blocks, 128, amh::tr5_smem_bytes(c->m.L, false), (cudaStream_t)cuda_stream>>>(
+        c->tm, states, B, d_out, omega_out, theta_out, phi_out);
+    AMH_CUDA(cudaGetLastError());
+    return AMH_OK;
+}
+
 amh_status amh_destroy(amh_ctx *c)
 {
     if (!c) return AMH_OK;
@@ -294,6 +428,7 @@ amh_status amh_destroy(amh_ctx *c)
     if (c->Elast) cudaFree(c->Elast);
     if (c->Ebd) cudaFree(c->Ebd);
     if (c->P) cudaFree(c->P);
+    for (double *q : c->tE) if (q) cudaFree(q);
     if (c->stage) cudaFree(c->stage);
     delete c;
     return AMH_OK;
@@ -302,6 +437,12 @@ amh_status amh_destroy(amh_ctx *c)
 static amh_status launch_energy(amh_ctx *c, const float *states, long long B, int k, int window, float *out, cudaStream_t st)
 {
     if (B == 0) return AMH_OK;
+    if (c->param == AMH_PARAM_TR5) {
+        const int blocks = (int)std::min<long long>(B, (long long)c->n_sm * 16);
+        amh::tr5_energy_kernel<<<blocks, 128, amh::tr5_smem_bytes(c->m.L, false), st>>>(c->tm, states, B, k, window, out);
+        AMH_CUDA(cudaGetLastError());
+        return AMH_OK;
+    }
     const size_t smem = sizeof(double) * 32 + sizeof(float) * 3 * (size_t)c->m.L;
     const int blocks = (int)std::min<long long>(B, (long long)c->n_sm * 64);
     amh::energy_kernel<<<blocks, 128, smem, st>>>(c->m, states, B, k, window, out);
@@ -337,6 +478,11 @@ amh_status amh_coords(amh_ctx *c, const float *states, long long B, float *cb_ou
     const int wpb = 4;
     const long long blocks = (B + wpb - 1) / wpb;
     if (blocks > 0x7fffffffLL) return fail(AMH_ERR_INVALID_ARG, "amh_coords: B too large");
+    if (c->param == AMH_PARAM_TR5) {
+        amh::tr5_coords_kernel<<<(int)blocks, 32 * wpb, 0, (cudaStream_t)cuda_stream>>>(c->tm, states, B, cb_out, atoms_out);
+        AMH_CUDA(cudaGetLastError());
+        return AMH_OK;
+    }
     amh::coords_kernel<<<(int)blocks, 32 * wpb, 0, (cudaStream_t)cuda_stream>>>(c->m, states, B, cb_out, atoms_out);
     AMH_CUDA(cudaGetLastError());
     return AMH_OK;
@@ -407,6 +553,18 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
 amh_status amh_launch_info(amh_ctx *c, long long B, int window, int *threads_per_chain, int *smem_bytes, int *ctas_per_sm, int *n_sm)
 {
     if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_launch_info: ctx is NULL");
+    if (c->param == AMH_PARAM_TR5) {
+        const int threads = 128;
+        if (threads_per_chain) *threads_per_chain = threads;
+        if (smem_bytes) *smem_bytes = (int)amh::tr5_smem_bytes(c->m.L, true);
+        if (n_sm) *n_sm = c->n_sm;
+        if (ctas_per_sm) {
+            int nb = 0;
+            AMH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, amh::tr5_sweep_kernel, threads, amh::tr5_smem_bytes(c->m.L, true)));
+            *ctas_per_sm = nb;
+        }
+        return AMH_OK;
+    }
     const SweepShape sh = choose_shape(c, std::max<long long>(B, 1), window);
     if (threads_per_chain) *threads_per_chain = 32 * sh.W;
     if (smem_bytes) *smem_bytes = (int)sh.smem;
@@ -422,6 +580,13 @@ amh_status amh_launch_info(amh_ctx *c, long long B, int window, int *threads_per
 amh_status amh_launch_shape(amh_ctx *c, long long B, int window, int *chains_per_cta, int *warps_per_chain, int *ring_cols, int *ring_rows)
 {
     if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_launch_shape: ctx is NULL");
+    if (c->param == AMH_PARAM_TR5) {
+        if (chains_per_cta) *chains_per_cta = 1;
+        if (warps_per_chain) *warps_per_chain = 4;
+        if (ring_cols) *ring_cols = 0;
+        if (ring_rows) *ring_rows = 0;
+        return AMH_OK;
+    }
     const SweepShape sh = choose_shape(c, std::max<long long>(B, 1), window);
     if (chains_per_cta) *chains_per_cta = sh.C;
     if (warps_per_chain) *warps_per_chain = sh.W;
@@ -487,6 +652,14 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
         if (a.first_hit) AMH_CUDA(cudaMemsetAsync(a.first_hit, 0xFF, sizeof(unsigned long long), st));   // -1 = none
     }
     if (B == 0) return AMH_OK;
+    if (c->param == AMH_PARAM_TR5) {
+        // config 3: one CTA per chain, one proposal at a time (amh_tr5.cuh)
+        const int threads = 128;
+        const long long ctas = std::min<long long>(B, (long long)c->n_sm * 8);
+        amh::tr5_sweep_kernel<<<(unsigned)ctas, threads, amh::tr5_smem_bytes(c->m.L, true), st>>>(c->tm, a);
+        AMH_CUDA(cudaGetLastError());
+        return AMH_OK;
+    }
     const SweepShape sh = choose_shape(c, B, sc->window);
     if (sh.smem > (size_t)c->max_smem)
         return fail(AMH_ERR_UNSUPPORTED, "amh_run: L = %d, window = %d, %d chains x %d warps need %zu B of shared memory, device allows %d",
