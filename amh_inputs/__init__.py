@@ -53,13 +53,13 @@ class Config:
 
 
 # BASELINE.json:8-12.  cfg 3 is the trRosetta2-style energy on the 5-slot state (n = 5 L; R25): 37 distance bins
-# over 2-20 A plus 24/24/12-bin orientation maps; it gives no sweep count (R11: 110 sweeps are used).
+# over 2-20 A plus 24/24/12-bin orientation maps; it gives no sweep count (R11: 33 sweeps = three cycles are used).
 CONFIGS = {
     0: Config("cfg0", L=64, B=32, n_sweeps=2200, n_global=1, n_local=10, window=8, cfg_seed=1000),
     1: Config("cfg1", L=128, B=1024, n_sweeps=10000, n_global=1, n_local=10, window=8, cfg_seed=1001),
     2: Config("cfg2", L=256, B=4096, n_sweeps=20000, n_global=1, n_local=10, window=12,
               t_start=10.0, t_end=0.1, cfg_seed=1002),
-    3: Config("cfg3", L=300, B=2048, n_sweeps=110, n_global=1, n_local=10, window=12, n_bins=37, d_lo=2.0, d_hi=20.0,
+    3: Config("cfg3", L=300, B=2048, n_sweeps=33, n_global=1, n_local=10, window=12, n_bins=37, d_lo=2.0, d_hi=20.0,
               cfg_seed=1003, slots=5),
     4: Config("cfg4", L=600, B=8192, n_sweeps=300, n_global=1, n_local=2, window=12,
               t_start=0.1, t_end=5.0, replicas=8, cfg_seed=1004),

@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py - AMH sampling rate (MH proposals/s summed over all chains) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference] [--per-config full|slice|off]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
         --master-port P bench.py --gpus N --steps K --warmup W
 
@@ -10,18 +10,22 @@ A step = one pass of the whole hot path over one batch: amh_run on a full config
 the seeded random start.  Inputs are synthetic (amh_inputs) and resident
 in HBM when the timed region starts; the e2e leg goes through amh_run_host with pinned host
 buffers.  Multi-GPU = chain sharding, no data-path collective: rank r
-runs chains [r*B, (r+1)*B), weak scaling.  Rank 0 prints ONE JSON line.
+runs chains [r*B, (r+1)*B), weak scaling; `--gpus N` without a launcher environment starts the N
+ranks itself (torch.distributed.run on 127.0.0.1).  Rank 0 prints ONE JSON line.  At N = 1 the line
+also carries `per_config`: every other config of BASELINE.json, one timed step each.
 
 --impl reference times the fp64 CPU oracle (oracle/) as it stands on the host cores, on a bounded
-sample of the same workload; it is the only place besides the cpu_baseline leg where this file
+sample of the same workload; it is the only place besides the cpu_baseline legs where this file
 executes anything under oracle/.
 """
 from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import re
+import socket
 import subprocess
 import sys
 import tempfile
@@ -37,22 +41,38 @@ import amh_inputs as gi  # noqa: E402
 
 METRIC = "mh_proposals_per_sec"
 UNIT = "proposals/s"
-LANE_OPS_PER_PAIR = 20          # fp32 lane-ops of one pair evaluation
+# Thread instructions of ONE pair evaluation in the built kernel (cuobjdump -sass of sweep_kernel<1,1,1>, the body of
+# local_new_sum; profiles/r2_sass_pair_eval.md): 9 FADD + 3 FMNMX + 2 FSEL + 1 FMUL + 4 FFMA + 1 MUFU.SQRT + 4 integer
+# (SHL, LOP3, IADD3, IADD) + 4 shared-memory loads (2 LDS.128 points, 2 LDS table entries) = 28.  (SURVEY.md 8(d) estimated 20.)
+LANE_OPS_PER_PAIR = 28
+LANE_OPS_BY_PIPE = {"fadd_fmnmx_fsel": 14, "ffma_fmul": 5, "mufu": 1, "int": 4, "lds": 4}
+LANE_OPS_DISTANCE = 8           # of those, what a pair beyond the last bin centre needs: 1 load, 3 FADD, 1 FMUL, 2 FFMA, 1 compare
+# config 3 (fp64): DFMA-class instructions of one six-term pair (three dihedrals, two angles, six interpolations): counted in
+# the SASS of tr5_sweep_kernel (profiles/r2_sass_pair_eval.md)
+LANE_OPS_PER_PAIR_TR5 = 640
 FP32_LANES_PER_SM = 128
+FP64_LANES_PER_SM = 64
 
 
 # ------------------------------------------------------------------------------------------------
-def pair_counts(L: int, w: int, min_sep: int = 3):
+def pair_counts(L: int, w: int, min_sep: int = 3, slots: int = 2):
     """Algorithmic pair evaluations per sweep: sum over k of the pairs that straddle
     the flipped bond, for a global and for a local sweep, and the all-pairs count of the sweep-end energy."""
     i = np.arange(L)[:, None]; j = np.arange(L)[None, :]
     sep_ok = (j - i) >= min_sep
     g = l = 0
-    for k in range(2 * L):
-        c = k // 2
-        split = c + (k & 1)
-        if k == 0 or k == 2 * L - 1:
-            continue
+    for k in range(slots * L):
+        c, slot = divmod(k, slots)
+        if slots == 2:
+            split = c + slot
+            if k == 0 or k == 2 * L - 1:
+                continue
+        else:
+            if slot >= 3:
+                continue
+            split = c + (1 if slot > 0 else 0)
+            if split <= 0 or split >= L:
+                continue
         cross = sep_ok & (i < split) & (j >= split)
         g += int(cross.sum())
         lo, hi = max(0, c - w), min(L - 1, c + w)
@@ -61,7 +81,7 @@ def pair_counts(L: int, w: int, min_sep: int = 3):
 
 
 def algorithmic_pair_evals(cfg: gi.Config) -> int:
-    g, l, allp = pair_counts(cfg.L, cfg.window)
+    g, l, allp = pair_counts(cfg.L, cfg.window, slots=cfg.slots)
     cyc = cfg.n_global + cfg.n_local
     full, rem = divmod(cfg.n_sweeps, cyc)
     n_g = full * cfg.n_global + min(rem, cfg.n_global)
@@ -78,16 +98,37 @@ def run_kwargs(cfg: gi.Config, B: int, chain_offset: int):
     return kw
 
 
+def start_states(cfg: gi.Config, B: int, seed: int, chain_offset: int = 0) -> np.ndarray:
+    if cfg.slots == 5:
+        return gi.initial_states_tr5(B, cfg.L, seed, chain_offset)
+    return gi.initial_states(B, cfg.n, seed=seed, chain_offset=chain_offset)
+
+
 def shard(cfg: gi.Config, rank: int, world: int):
     """Chain sharding: rank r runs chains [r B, (r+1) B) of a world*B batch - weak scaling,
     no data-path collective.  Returns (chain_offset, start states, run kwargs) of this rank."""
     off = rank * cfg.B
-    return off, gi.initial_states(cfg.B, cfg.n, seed=1, chain_offset=off), run_kwargs(cfg, cfg.B, off)
+    return off, start_states(cfg, cfg.B, 1, off), run_kwargs(cfg, cfg.B, off)
 
 
 def job_rate(world: int, proposals_per_rank: int, steps: int, max_total_ms: float) -> float:
     """Whole-job proposals/s: the units all ranks processed / the slowest rank's device time."""
     return world * proposals_per_rank * steps / (max_total_ms * 1e-3)
+
+
+def free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def spawn_ranks(n: int, argv) -> int:
+    """`bench.py --gpus N` without a launcher environment: start the N ranks on this node (one per GPU) with
+    torch.distributed.run on 127.0.0.1 and return its exit code."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n),
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + list(argv)
+    env = dict(os.environ, NCCL_DEBUG=os.environ.get("NCCL_DEBUG", "INFO"), NCCL_DEBUG_SUBSYS=os.environ.get("NCCL_DEBUG_SUBSYS", "INIT"))
+    return subprocess.call(cmd, env=env)
 
 
 class ClockSampler:
@@ -140,12 +181,13 @@ def measured_peaks():
         return {}
 
 
-def profiled_traffic(cfg_name: str):
-    """dram bytes per launch of the sweep kernel from the committed ncu --set full summary, or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.txt")
+def profiled_per_proposal(cfg_name: str, key: str):
+    """bytes per proposal of the sweep kernel from the committed ncu --set full summaries (profiles/r2_traffic.txt:
+    `<cfg> <key> = <value>`), or None.  key = dram_bytes_per_proposal | l2_bytes_per_proposal."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.txt")
     try:
         for line in open(path):
-            m = re.match(r"\s*%s\s+sweep_kernel\s+dram_bytes_per_launch\s*=\s*([0-9.eE+]+)" % re.escape(cfg_name), line)
+            m = re.match(r"\s*%s\s+%s\s*=\s*([0-9.eE+-]+)" % (re.escape(cfg_name), re.escape(key)), line)
             if m:
                 return float(m.group(1))
     except OSError:
@@ -154,24 +196,41 @@ def profiled_traffic(cfg_name: str):
 
 
 # ------------------------------------------------------------------------------------------------
-def oracle_leg(cfg: gi.Config, steps: int = 1, warmup: int = 0, target_s: float = 15.0):
-    """The fp64 oracle, as it stands, on the host cores, on a bounded sample of the workload: the first 64 chains
-    of the batch for as many whole cycles of the schedule as fit in about `target_s` seconds of wall time per step
-    (sized from a two-cycle calibration run; at least two cycles, at most the config's sweep count)."""
+def oracle_model(cfg: gi.Config):
+    """The config's energy model in the oracle, from the oracle's own reference geometry."""
     import oracle
     oracle.build()
+    edges = gi.bin_edges(cfg.n_bins, cfg.d_lo, cfg.d_hi)
+    if cfg.slots == 5:
+        ref = gi.reference_torsions_tr5(cfg.L, cfg.cfg_seed)
+        D, OM, TH, PH = oracle.tr5_pair_geometry(ref)
+        return oracle.TR5Model(gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi), edges,
+                               gi.periodic_map_from_values(OM, 24, -math.pi, math.pi, True),
+                               gi.periodic_map_from_values(TH, 24, -math.pi, math.pi, True),
+                               gi.periodic_map_from_values(PH, 12, 0.0, math.pi, False))
     ref = gi.reference_torsions(cfg.L, cfg.cfg_seed)
     CB = oracle.coords(ref)[3]
     D = np.linalg.norm(CB[:, None] - CB[None], axis=-1)
-    m = oracle.Model(gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi), gi.bin_edges(cfg.n_bins, cfg.d_lo, cfg.d_hi))
-    chains = min(cfg.B, 64)
-    s0 = gi.initial_states(chains, cfg.n, seed=1)
+    return oracle.Model(gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi), edges)
+
+
+def oracle_leg(cfg: gi.Config, steps: int = 1, warmup: int = 0, target_s: float = 15.0, max_chains: int = 64):
+    """The fp64 oracle, as it stands, on the host cores, on a bounded sample of the workload: the first chains
+    of the batch for as many whole cycles of the schedule as fit in about `target_s` seconds of wall time per step
+    (sized from a calibration run; at least one cycle, at most the config's sweep count)."""
+    import oracle
+    m = oracle_model(cfg)
+    chains = min(cfg.B, max_chains)
+    s0 = start_states(cfg, chains, 1)
     kw = run_kwargs(cfg, chains, 0)
     cyc = cfg.n_global + cfg.n_local
+    ncal = 1 if cfg.L > 256 or cfg.slots == 5 else 2
+    if cfg.L > 256 or cfg.slots == 5:
+        chains = min(chains, max(oracle.num_threads(), 1)); s0 = s0[:chains]; kw = run_kwargs(cfg, chains, 0)
     t0 = time.perf_counter()
-    m.run(s0, min(cfg.n_sweeps, 2 * cyc), **kw)
-    t_cal = (time.perf_counter() - t0) / 2.0
-    sweeps = int(min(cfg.n_sweeps, cyc * max(2, int(target_s / max(t_cal, 1e-6)))))
+    m.run(s0, min(cfg.n_sweeps, ncal * cyc), **kw)
+    t_cal = (time.perf_counter() - t0) / ncal
+    sweeps = int(min(cfg.n_sweeps, cyc * max(1, int(target_s / max(t_cal, 1e-6)))))
     times = []
     for it in range(warmup + steps):
         t0 = time.perf_counter()
@@ -191,18 +250,144 @@ def oracle_threshold(cfg: gi.Config, runs: int = 10, proposals: int = 100000):
     runs `runs` single chains of `proposals` proposals each under the config's schedule, one core per chain; E* = mean
     of their minimum sweep-end energies, cpu_s = wall time of those runs."""
     import oracle
-    oracle.build()
-    ref = gi.reference_torsions(cfg.L, cfg.cfg_seed)
-    CB = oracle.coords(ref)[3]
-    D = np.linalg.norm(CB[:, None] - CB[None], axis=-1)
-    m = oracle.Model(gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi), gi.bin_edges(cfg.n_bins, cfg.d_lo, cfg.d_hi))
+    m = oracle_model(cfg)
     sweeps = max(1, -(-proposals // cfg.n))
-    s0 = gi.initial_states(runs, cfg.n, seed=1)
+    s0 = start_states(cfg, runs, 1)
     t0 = time.perf_counter()
     r = m.run(s0, sweeps, **run_kwargs(cfg, runs, 0))
     dt = time.perf_counter() - t0
     return dict(threshold=float(np.mean(r["best_energy"])), cpu_s=dt, cpu_runs=runs, cpu_sweeps_per_run=sweeps,
                 cpu_cores=min(runs, oracle.num_threads()))
+
+
+# ------------------------------------------------------------------------------------------------
+class Workload:
+    """One config on the CUDA path: context (tables built from the CUDA path's own reference geometry), start states."""
+
+    def __init__(self, pkg, torch, cfg: gi.Config, rank: int, world: int, launch_over=None):
+        self.pkg, self.torch, self.cfg = pkg, torch, cfg
+        L = cfg.L
+        edges = gi.bin_edges(cfg.n_bins, cfg.d_lo, cfg.d_hi)
+        opts = pkg.default_options(**launch_over) if launch_over else None
+        if cfg.slots == 5:
+            ref = gi.reference_torsions_tr5(L, cfg.cfg_seed)
+            flat = [np.full((L, L, nb), 1.0 / nb, np.float32) for nb in (cfg.n_bins, 24, 24, 12)]
+            g0 = pkg.AMH(flat[0], edges, orientation=flat[1:])
+            D, OM, TH, PH = [x[0].cpu().numpy() for x in g0.pair_geometry(torch.from_numpy(ref[None]).cuda())]
+            g0.close()
+            self.g = pkg.AMH(gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi), edges, opts,
+                             orientation=(gi.periodic_map_from_values(OM, 24, -math.pi, math.pi, True),
+                                          gi.periodic_map_from_values(TH, 24, -math.pi, math.pi, True),
+                                          gi.periodic_map_from_values(PH, 12, 0.0, math.pi, False)))
+        else:
+            # reference geometry from the CUDA path itself (a throw-away context with a flat table)
+            g0 = pkg.AMH(np.full((L, L, cfg.n_bins), 1.0 / cfg.n_bins, np.float32), edges)
+            ref = gi.reference_torsions(L, cfg.cfg_seed)
+            cb = g0.coords(torch.from_numpy(ref[None]).cuda())[0].double().cpu().numpy()
+            g0.close()
+            D = np.linalg.norm(cb[:, None] - cb[None], axis=-1)
+            self.g = pkg.AMH(gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi), edges, opts)
+        self.chain_offset, s0_np, self.kw = shard(cfg, rank, world)
+        self.s0_host = torch.from_numpy(s0_np).pin_memory()
+        self.s0_dev = self.s0_host.cuda()
+        self.states = torch.empty_like(self.s0_dev)
+        if "per_chain_T" in self.kw:
+            self.kw["per_chain_T"] = torch.from_numpy(self.kw["per_chain_T"]).cuda()
+        self.info = self.g.launch_info(cfg.B, cfg.window)
+
+    def kernel_label(self) -> str:
+        i = self.info
+        if self.cfg.slots == 5:
+            return "amh::tr5_sweep_kernel (fp64, one CTA of %d threads per chain)" % i["threads_per_chain"]
+        return ("amh::sweep_kernel<SG=%d, RING=%d, CB64=%d>: %d chains x %d warps per CTA, %d local proposals per pass, %d lanes each"
+                % (i["spec_global"], i["ring"], i["cb64"], i["chains_per_cta"], i["warps_per_chain"], i["nspec"], i["lanes_per_step"]))
+
+    def launch_dict(self) -> dict:
+        i = self.info
+        return dict(kernel=self.kernel_label(), threads_per_chain=i["threads_per_chain"], chains_per_cta=i["chains_per_cta"],
+                    ring_cols=i["ring_cols"], ring_rows=i["ring_rows"], smem_bytes_per_cta=i["smem_bytes"],
+                    ctas_resident_per_sm=i["ctas_per_sm"])
+
+    def run(self, sweeps=None, want=("energy", "best_energy"), **over):
+        return self.g.run(self.states, self.cfg.n_sweeps if sweeps is None else sweeps, want=want, **dict(self.kw, **over))
+
+    def reset(self):
+        self.states.copy_(self.s0_dev)
+
+    def near_fraction(self, states) -> float:
+        """fraction of the pairs j - i >= 3 of (a sample of) these states that lie below the last bin centre, i.e. that need
+        more than their distance (measured with torch on the C-betas amh_coords returns; reporting only)"""
+        torch, cfg = self.torch, self.cfg
+        pick = states[:: max(1, states.shape[0] // 64)][:64]
+        cb = self.g.coords(pick).double()
+        d = torch.cdist(cb, cb)
+        i = torch.arange(cfg.L, device=d.device)
+        mask = (i[None, :] - i[:, None]) >= 3
+        c_last = cfg.d_hi - 0.5 * (cfg.d_hi - cfg.d_lo) / cfg.n_bins
+        return float(((d < c_last) & mask[None]).sum().item()) / float(mask.sum().item() * d.shape[0])
+
+    def roofline(self, ms_per_step: float, n_sm: int, sm_max_mhz: float, peaks: dict, l2_peak_gbs, gather_peak) -> dict:
+        cfg = self.cfg
+        pair_evals = algorithmic_pair_evals(cfg)
+        fp64 = cfg.slots == 5
+        ops = LANE_OPS_PER_PAIR_TR5 if fp64 else LANE_OPS_PER_PAIR
+        lanes = FP64_LANES_PER_SM if fp64 else FP32_LANES_PER_SM
+        peak = n_sm * lanes * sm_max_mhz * 1e6 / 1e9          # Glane-op/s
+        achieved = pair_evals * ops / (ms_per_step * 1e-3) / 1e9
+        dram = profiled_per_proposal(cfg.name, "dram_bytes_per_proposal")
+        l2b = profiled_per_proposal(cfg.name, "l2_bytes_per_proposal")
+        r = dict(bound="alu", achieved=achieved, peak=peak, unit="Glane-op/s", frac=achieved / peak,
+                 traffic=(dram * cfg.proposals) if dram is not None else None,
+                 traffic_source="dram bytes per proposal of the ncu --set full capture of this config's kernel (profiles/r2_traffic.txt) x proposals per launch",
+                 kernel=self.kernel_label(), pair_evals_per_launch=pair_evals, lane_ops_per_pair_eval=ops,
+                 lane_ops_by_pipe=None if fp64 else LANE_OPS_BY_PIPE, pair_evals_per_s=pair_evals / (ms_per_step * 1e-3),
+                 peak_source="derived: %d SMs x %d %s lanes x %.0f MHz (clocks.max.sm)" % (n_sm, lanes, "fp64" if fp64 else "fp32", sm_max_mhz),
+                 hbm_gbs_measured=peaks.get("hbm_gbs"))
+        if not fp64:
+            # a more conservative count: every pair needs its distance (8 lane-ops); only a near pair - and every in-window pair
+            # of a local proposal, where no far test is made - needs the other 20.  near fraction = the smaller of the start
+            # and the final states' (the states in between are at least as compact as the random start).
+            f = min(self.near_fraction(self.s0_dev), self.near_fraction(self.states))
+            gsum, lsum, allp = pair_counts(cfg.L, cfg.window, slots=cfg.slots)
+            cyc = cfg.n_global + cfg.n_local
+            full, rem = divmod(cfg.n_sweeps, cyc)
+            n_g = full * cfg.n_global + min(rem, cfg.n_global)
+            n_l = cfg.n_sweeps - n_g
+            ops = cfg.B * (n_l * lsum * LANE_OPS_PER_PAIR + (n_g * gsum + cfg.n_sweeps * allp) * (LANE_OPS_DISTANCE + f * (LANE_OPS_PER_PAIR - LANE_OPS_DISTANCE)))
+            r["frac_distance_weighted"] = ops / (ms_per_step * 1e-3) / 1e9 / peak
+            r["near_fraction"] = f
+            r["note"] = ("frac counts EVERY straddling pair at the %d lane-ops of a full evaluation (SURVEY.md 8(d)'s unit); the kernel skips pairs "
+                         "beyond the last bin centre exactly (their term is 0), so frac can exceed 1 where most pairs are far (config 4). "
+                         "frac_distance_weighted charges a far pair only its distance test (%d lane-ops)." % (LANE_OPS_PER_PAIR, LANE_OPS_DISTANCE))
+        ipp = profiled_per_proposal(cfg.name, "thread_inst_per_proposal")
+        if ipp is not None:
+            r["executed_thread_inst_per_algorithmic_pair"] = ipp * cfg.proposals / pair_evals
+        if l2_peak_gbs:
+            a = (l2b * cfg.proposals / (ms_per_step * 1e-3) / 1e9) if l2b is not None else None
+            r["l2"] = dict(achieved=a, peak=l2_peak_gbs, unit="GB/s", frac=(a / l2_peak_gbs) if a is not None else None,
+                           peak_source="amh_probe_l2_read measured in this run: read-only sweep of a %d MB buffer by every SM, L1 bypassed"
+                                       % (48 if cfg.L < 512 else 92),
+                           achieved_source="lts__t_bytes per proposal of the ncu capture (profiles/r2_traffic.txt) x proposals / this run's time")
+        if gather_peak:
+            r["gather_ceiling"] = dict(peak=gather_peak, unit="8-byte gathers/s",
+                                       note="amh_probe_gather measured in this run: the near-pair look-ups of the global phase cannot exceed it")
+        return r
+
+
+def time_steps(torch, wl: Workload, steps: int, warmup: int, flush, stream, barrier, run_step):
+    for _ in range(warmup):
+        wl.reset(); run_step()
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    res = None
+    for a, b in ev:
+        flush.fill_(1)                                  # L2 flush between timed iterations (outside the events)
+        wl.reset()
+        a.record(stream)
+        res = run_step()
+        b.record(stream)
+    barrier()
+    return sum(a.elapsed_time(b) for a, b in ev), res
 
 
 def main():
@@ -212,6 +397,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, choices=sorted(gi.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--per-config", default="full", choices=["full", "slice", "off"],
+                    help="N = 1 only: after the headline, one timed step of every other config (full = the whole config; slice = a few cycles)")
     ap.add_argument("--sweeps", type=int, default=0, help="override the config's sweep count (experiments only; the line says so)")
     ap.add_argument("--chains", type=int, default=0, help="override the config's chain count (experiments only)")
     ap.add_argument("--warps-per-chain", type=int, default=0)
@@ -223,7 +410,12 @@ def main():
     ap.add_argument("--exchange", action="store_true", help="configs with temperature replicas: amh_run_pt (replica exchange after every cycle, NEXT-3) instead of amh_run; the line says so")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--dry-run", action="store_true", help="launcher / sharding check without a GPU: gloo, no kernels, the line reports the shards")
     args = ap.parse_args()
+
+    # `--gpus N` without a launcher environment: start the N ranks ourselves
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1 and args.impl == "ours":
+        sys.exit(spawn_ranks(args.gpus, sys.argv[1:]))
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -233,11 +425,16 @@ def main():
     if overridden:
         import dataclasses
         cfg = dataclasses.replace(cfg, n_sweeps=args.sweeps or cfg.n_sweeps, B=args.chains or cfg.B)
-    workload = dict(workload=cfg.name + ("-override" if overridden else ""), L=cfg.L, chains_per_gpu=cfg.B, sweeps=cfg.n_sweeps,
-                    schedule="%d global : %d local" % (cfg.n_global, cfg.n_local), window=cfg.window,
-                    temperature=("per-chain %g..%g x%d" % (cfg.t_start, cfg.t_end, cfg.replicas)) if cfg.replicas
-                    else ("%g -> %g geometric" % (cfg.t_start, cfg.t_end) if cfg.t_start != cfg.t_end else "%g" % cfg.t_start),
-                    n_bins=cfg.n_bins, proposal="uniform", parallelism="chains sharded x%d" % world)
+
+    def workload_dict(c: gi.Config, over=False):
+        return dict(workload=c.name + ("-override" if over else ""), L=c.L, chains_per_gpu=c.B, sweeps=c.n_sweeps,
+                    variables_per_chain=c.n, schedule="%d global : %d local" % (c.n_global, c.n_local), window=c.window,
+                    temperature=("per-chain %g..%g x%d" % (c.t_start, c.t_end, c.replicas)) if c.replicas
+                    else ("%g -> %g geometric" % (c.t_start, c.t_end) if c.t_start != c.t_end else "%g" % c.t_start),
+                    n_bins=c.n_bins, proposal="uniform", parallelism="chains sharded x%d" % world,
+                    l2="flushed between timed steps (256 MiB write)",
+                    step="amh_run over the full config from the seeded random start")
+    workload = workload_dict(cfg, overridden)
 
     # ---------------- reference arm: the oracle on the host cores --------------------------------
     if args.impl == "reference":
@@ -249,6 +446,29 @@ def main():
                     dtype="f64", data="synthetic", config=workload, cpu_baseline=cb,
                     e2e=dict(value=cb["value"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
         print(json.dumps(line))
+        return
+
+    # ---------------- launcher / sharding check without a GPU ------------------------------------
+    if args.dry_run:
+        import torch
+        import torch.distributed as dist
+        if world > 1:
+            dist.init_process_group("gloo")
+        off, s0, kw = shard(cfg, rank, world)
+        mine = torch.tensor([rank, off, off + cfg.B, int(np.float64(s0.sum()) * 1000) % 1000003], dtype=torch.int64)
+        allr = [torch.zeros_like(mine) for _ in range(world)]
+        if world > 1:
+            dist.all_gather(allr, mine)
+        else:
+            allr = [mine]
+        tmax = torch.tensor([1.0 + rank], dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        if rank == 0:
+            print(json.dumps(dict(metric=METRIC, dry_run=True, n_gpus=len(allr), value=job_rate(world, cfg.proposals, 1, float(tmax.item())),
+                                  shards=[[int(x) for x in r] for r in allr], config=workload)))
+        if world > 1:
+            dist.destroy_process_group()
         return
 
     # ---------------- our arm --------------------------------------------------------------------
@@ -268,41 +488,27 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    L, B, n = cfg.L, cfg.B, cfg.n
-    edges = gi.bin_edges(cfg.n_bins, cfg.d_lo, cfg.d_hi)
-    # reference geometry from the CUDA path itself (a throw-away context with a flat table)
-    g0 = pkg.AMH(np.full((L, L, cfg.n_bins), 1.0 / cfg.n_bins, np.float32), edges)
-    ref = gi.reference_torsions(L, cfg.cfg_seed)
-    cb = g0.coords(torch.from_numpy(ref[None]).cuda())[0].double().cpu().numpy()
-    g0.close()
-    D = np.linalg.norm(cb[:, None] - cb[None], axis=-1)
-    p = gi.distogram_from_distances(D, n_bins=cfg.n_bins, lo=cfg.d_lo, hi=cfg.d_hi)
-    g = pkg.AMH(p, edges, pkg.default_options(warps_per_chain=args.warps_per_chain, chains_per_cta=args.chains_per_cta,
-                                               spec_local=args.spec_local, ring_cols=args.ring_cols,
-                                               lanes_per_step=args.lanes_per_step, spec_global=args.spec_global))
-    del p
-    chain_offset, s0_np, kw = shard(cfg, rank, world)
-    s0_host = torch.from_numpy(s0_np).pin_memory()
-    s0_dev = s0_host.cuda()
-    states = torch.empty_like(s0_dev)
-    if "per_chain_T" in kw:
-        kw["per_chain_T"] = torch.from_numpy(kw["per_chain_T"]).cuda()
+    launch_over = dict(warps_per_chain=args.warps_per_chain, chains_per_cta=args.chains_per_cta, spec_local=args.spec_local,
+                       ring_cols=args.ring_cols, lanes_per_step=args.lanes_per_step, spec_global=args.spec_global)
+    wl = Workload(pkg, torch, cfg, rank, world, launch_over)
+    g, kw, states, B, n = wl.g, wl.kw, wl.states, cfg.B, cfg.n
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
     stream = torch.cuda.current_stream()
-    info = g.launch_info(B, cfg.window)
+    info = wl.info
 
     exchange = bool(args.exchange and cfg.replicas)
     tts = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not exchange:
-        tts = oracle_threshold(cfg)
-        kw["energy_threshold"] = tts["threshold"]
+        tts = oracle_threshold(cfg) if cfg.slots == 2 and cfg.L <= 256 else None
+        if tts is not None:
+            kw["energy_threshold"] = tts["threshold"]
 
     if exchange:
         args.no_e2e = True                                   # the exchange run is an experiment line: device-timed rate only
         # replica exchange: one amh_run per cycle + amh_exchange, enqueued by amh_run_pt; temperatures reset every step
         T0 = kw.pop("per_chain_T")
         Tcur = T0.clone()
-        ptkw = dict(n_global=cfg.n_global, n_local=cfg.n_local, window=cfg.window, seed=kw["seed"], chain_offset=chain_offset)
+        ptkw = dict(n_global=cfg.n_global, n_local=cfg.n_local, window=cfg.window, seed=kw["seed"], chain_offset=wl.chain_offset)
         n_cycles = cfg.n_sweeps // (cfg.n_global + cfg.n_local)
         workload["exchange"] = "amh_run_pt: %d cycles, exchange after each, groups of %d" % (n_cycles, cfg.replicas)
 
@@ -310,28 +516,11 @@ def main():
         if exchange:
             Tcur.copy_(T0)
             return g.run_pt(states, n_cycles, Tcur, cfg.replicas, **ptkw)
-        return g.run(states, cfg.n_sweeps, want=("energy", "best_energy"), **kw)
+        return wl.run()
 
-    def one_step():
-        states.copy_(s0_dev)
-        return run_step()
-
-    for _ in range(args.warmup):
-        one_step()
-    barrier()
     sampler = ClockSampler(local_rank) if rank == 0 else None
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    launches = 0
-    res = None
-    for a, b in ev:
-        flush.fill_(1)                                  # L2 flush between timed iterations (outside the events)
-        states.copy_(s0_dev)
-        a.record(stream)
-        res = run_step()
-        b.record(stream)
-        launches += (2 * n_cycles) if exchange else 1
-    barrier()
-    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    total_ms, res = time_steps(torch, wl, args.steps, args.warmup, flush, stream, barrier, run_step)
+    launches = args.steps * ((2 * n_cycles) if exchange else 1)
     clocks = sampler.stop() if sampler else None
     tmax = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
     if dist is not None:
@@ -343,30 +532,45 @@ def main():
     best = float(res["best_energy"].min().item()) if res is not None else None
     if tts is not None:
         hit = int(res["first_hit_sweep"].item())
-        tts.update(first_hit_sweep=hit, gpu_s=(ms_per_step * 1e-3 * (hit + 1) / cfg.n_sweeps) if hit >= 0 else None,
+        kw.pop("energy_threshold")
+
+        def timed_to(sweeps, seed):
+            """device time of an amh_run of `sweeps` sweeps from the seeded start (the time to reach the threshold, measured)"""
+            s = wl.s0_dev if seed == 1 else torch.from_numpy(start_states(cfg, B, seed, wl.chain_offset)).cuda()
+            states.copy_(s)
+            a2, b2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a2.record(stream)
+            rr = g.run(states, sweeps, want=("energy",), **dict(kw, seed=seed, energy_threshold=tts["threshold"]))
+            b2.record(stream)
+            torch.cuda.synchronize()
+            return a2.elapsed_time(b2) * 1e-3, int(rr["first_hit_sweep"].item())
+        gpu_s = None
+        if hit >= 0:
+            timed_to(hit + 1, 1)
+            gpu_s, h2 = timed_to(hit + 1, 1)
+            assert h2 == hit
+        tts.update(first_hit_sweep=hit, gpu_s=gpu_s,
                    protocol="E* = mean over 10 oracle chains (100,000 proposals each, this config's schedule) of the minimum "
-                            "sweep-end energy; gpu_s = step time x (first sweep at whose end some chain of the batch has V <= E*, "
-                            "+ 1) / sweeps; cpu_s = wall time of the oracle runs, one core per chain")
-        # nine more seeds (PAPER.md:184-188 takes means over repeated runs; median over 10 seeds),
-        # each run only long enough to see its hit
-        hits = [hit]
+                            "sweep-end energy; gpu_s = MEASURED device time (CUDA events) of an amh_run of exactly first_hit_sweep + 1 sweeps "
+                            "from the same start, first_hit_sweep = first sweep at whose end some chain of the batch has V <= E*; "
+                            "cpu_s = wall time of the oracle runs, one core per chain")
+        # nine more seeds (PAPER.md:184-188 takes means over repeated runs; SURVEY.md 8(d): median over 10 seeds)
+        hits, times = [hit], [gpu_s]
         if hit >= 0:
             short = int(min(cfg.n_sweeps, 8 * (hit + 1) + 4 * (cfg.n_global + cfg.n_local)))
             for seed in range(2, 11):
-                states.copy_(torch.from_numpy(gi.initial_states(B, n, seed=seed, chain_offset=chain_offset)).cuda())
-                rr = g.run(states, short, want=("energy",), **dict(kw, seed=seed))
-                hits.append(int(rr["first_hit_sweep"].item()))
-            ok = sorted(h for h in hits if h >= 0)
-            med = ok[len(ok) // 2] if len(ok) == len(hits) else None
-            tts.update(first_hit_sweeps_10_seeds=hits, gpu_s_median=(ms_per_step * 1e-3 * (med + 1) / cfg.n_sweeps) if med is not None else None)
-        tts["speedup_vs_oracle"] = (tts["cpu_s"] / tts["gpu_s"]) if tts["gpu_s"] else None
-        kw.pop("energy_threshold")
+                _, h = timed_to(short, seed)
+                hits.append(h)
+                times.append(timed_to(h + 1, seed)[0] if h >= 0 else None)
+            ok = sorted(x for x in times if x is not None)
+            tts.update(first_hit_sweeps_10_seeds=hits, gpu_s_10_seeds=times, gpu_s_median=ok[len(ok) // 2] if len(ok) == len(times) else None)
+        tts["speedup_vs_oracle_chain"] = (tts["cpu_s"] / tts["gpu_s"]) if tts["gpu_s"] else None
+        tts["note"] = "speedup is over the deliberately slow fp64 oracle (full rebuild + full re-sum per proposal), not over a tuned CPU implementation"
 
     # ---------------- global-only and local-only rates (SURVEY.md 8(d)), short runs from the final states ----------
     phase_rates = None
     if rank == 0 and world == 1 and not exchange:
         phase_rates = {}
-        cyc = cfg.n_global + cfg.n_local
         for name, (ng, nl, sw) in (("global_only", (1, 0, max(2, 2 * cfg.n_global))), ("local_only", (0, 1, max(10, 2 * cfg.n_local)))):
             pk = dict(kw, n_global=ng, n_local=nl, sweep_offset=cfg.n_sweeps)
             tmp = states.clone()
@@ -380,15 +584,16 @@ def main():
     # ---------------- e2e: the same step through amh_run_host, pinned host buffers ----------------
     e2e = None
     if not args.no_e2e:
-        hs = torch.empty_like(s0_host).pin_memory()
+        e2e_steps = min(args.steps, 5)
+        hs = torch.empty_like(wl.s0_host).pin_memory()
         hkw = dict(kw)
         if "per_chain_T" in hkw:
             hkw["per_chain_T"] = hkw["per_chain_T"].cpu().numpy()
-        hs.copy_(s0_host); g.run_host(hs.numpy(), cfg.n_sweeps, **hkw)         # warm-up (staging arena)
+        hs.copy_(wl.s0_host); g.run_host(hs.numpy(), cfg.n_sweeps, **hkw)         # warm-up (staging arena)
         barrier()
         t0 = time.perf_counter()
-        for _ in range(args.steps):
-            hs.copy_(s0_host)
+        for _ in range(e2e_steps):
+            hs.copy_(wl.s0_host)
             rh = g.run_host(hs.numpy(), cfg.n_sweeps, **hkw)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
@@ -397,8 +602,8 @@ def main():
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
         h2d = B * n * 4 + (B * 4 if cfg.replicas else 0)
         d2h = B * n * 4 + 2 * B * 4
-        e2e = dict(value=props_per_step * args.steps / float(te.item()), unit=UNIT, h2d_bytes_per_step=h2d,
-                   d2h_bytes_per_step=d2h, api="amh_run_host (pinned host buffers; copies inside the timed region)",
+        e2e = dict(value=props_per_step * e2e_steps / float(te.item()), unit=UNIT, h2d_bytes_per_step=h2d,
+                   d2h_bytes_per_step=d2h, steps=e2e_steps, api="amh_run_host (pinned host buffers; copies inside the timed region)",
                    best_energy=float(rh["best_energy"].min()))
 
     if rank != 0:
@@ -406,30 +611,53 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---------------- roofline of the dominant kernel (sweep_kernel, one launch per step) ---------
+    # ---------------- ceilings measured in this run, roofline of the dominant kernel (one launch per step) ---------
     peaks = measured_peaks()
     sm_max_mhz = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
-    peak = info["n_sm"] * FP32_LANES_PER_SM * sm_max_mhz * 1e6 / 1e9          # Glane-op/s
-    pair_evals = algorithmic_pair_evals(cfg)
-    achieved = pair_evals * LANE_OPS_PER_PAIR / (ms_per_step * 1e-3) / 1e9
-    roofline = dict(bound="alu", achieved=achieved, peak=peak, unit="Glane-op/s", frac=achieved / peak,
-                    traffic=profiled_traffic(cfg.name), kernel="amh::sweep_kernel<SG, RING> (one of four variants, chosen per launch)",
-                    pair_evals_per_launch=pair_evals, lane_ops_per_pair_eval=LANE_OPS_PER_PAIR,
-                    pair_evals_per_s=pair_evals / (ms_per_step * 1e-3),
-                    peak_source="derived: %d SMs x 128 fp32 lanes x %.0f MHz (clocks.max.sm)" % (info["n_sm"], sm_max_mhz),
-                    hbm_gbs_measured=peaks.get("hbm_gbs"))
+    l2_48 = pkg.probe_l2_read(48 << 20, 20)
+    l2_92 = pkg.probe_l2_read(92 << 20, 12)
+    gather = pkg.probe_gather(64 << 20, 5)
+    ceilings = dict(l2_read_gbs_48mb=l2_48, l2_read_gbs_92mb=l2_92, gathers_per_s_64mb=gather, hbm_gbs_measured=peaks.get("hbm_gbs"),
+                    source="amh_probe_l2_read / amh_probe_gather in this run; hbm from MEASURED_PEAKS.json")
+    roofline = wl.roofline(ms_per_step, info["n_sm"], sm_max_mhz, peaks, l2_92 if cfg.L >= 512 else l2_48, gather)
+    launch_headline = dict(wl.launch_dict(), best_energy=best)
     cpu_baseline = None
     if not args.no_cpu_baseline:
         cpu_baseline, _ = oracle_leg(cfg)
 
-    workload.update(l2="flushed between timed steps (256 MiB write)", threads_per_chain=info["threads_per_chain"],
-                    chains_per_cta=info["chains_per_cta"], ring_cols=info["ring_cols"], ring_rows=info["ring_rows"],
-                    smem_bytes_per_cta=info["smem_bytes"], ctas_resident_per_sm=info["ctas_per_sm"],
-                    step="amh_run over the full config from the seeded random start", best_energy=best)
+    # ---------------- every other config, one timed step each (N = 1) -------------------------------------------------
+    per_config = None
+    if world == 1 and args.per_config != "off" and not overridden and not exchange:
+        per_config = {}
+        for cid in sorted(gi.CONFIGS):
+            if cid == args.config:
+                continue
+            c2 = gi.CONFIGS[cid]
+            sliced = args.per_config == "slice" and c2.proposals > 2e9
+            if sliced:
+                import dataclasses
+                c2 = dataclasses.replace(c2, n_sweeps=4 * (c2.n_global + c2.n_local))
+            del wl.g
+            torch.cuda.empty_cache()
+            wl = Workload(pkg, torch, c2, 0, 1)
+            smp = ClockSampler(local_rank)
+            wl.reset(); wl.run(sweeps=min(c2.n_sweeps, 2 * (c2.n_global + c2.n_local)))      # warm-up: tables into L2, code loaded
+            ms, r2 = time_steps(torch, wl, 1, 0, flush, stream, barrier, wl.run)
+            ck = smp.stop()
+            entry = dict(value=c2.proposals / (ms * 1e-3), unit=UNIT, ms_per_step=ms, steps=1, warmup="2 cycles",
+                         dtype="f64" if c2.slots == 5 else "f32",
+                         config=workload_dict(c2, sliced), launch=wl.launch_dict(), clocks=ck,
+                         best_energy=float(r2["best_energy"].min().item()),
+                         roofline=wl.roofline(ms, info["n_sm"], sm_max_mhz, peaks, l2_92 if c2.L >= 512 else l2_48, gather))
+            if not args.no_cpu_baseline:
+                entry["cpu_baseline"] = oracle_leg(c2, target_s=4.0, max_chains=16)[0]
+            per_config[c2.name] = entry
+
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
-                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
-                data="synthetic", config=workload, clocks=clocks, e2e=e2e, gpu_launches=launches,
-                roofline=roofline, cpu_baseline=cpu_baseline, time_to_threshold=tts, phase_rates=phase_rates)
+                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64" if cfg.slots == 5 else "f32",
+                data="synthetic", config=workload, launch=launch_headline, clocks=clocks, e2e=e2e, gpu_launches=launches,
+                roofline=roofline, ceilings=ceilings, cpu_baseline=cpu_baseline, time_to_threshold=tts, phase_rates=phase_rates,
+                per_config=per_config)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

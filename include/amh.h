@@ -272,6 +272,23 @@ amh_status amh_launch_shape(amh_ctx *ctx, long long B, int window, int *chains_p
 amh_status amh_philox_test(const unsigned int *ctr, const unsigned int *key, unsigned int *out,
                            long long count, void *cuda_stream);
 
+/* Measurement hooks (SURVEY.md 8(d) "BW_L2 is not in MEASURED_PEAKS.json - measure it"): the two
+ * memory ceilings of the pair loops on the current device.  Both allocate a scratch buffer, run their kernel `reps` times
+ * (after one warm-up), time it with CUDA events on the stream, free the buffer and synchronise.  Host outputs.
+ *   amh_probe_l2_read   every SM sweeps a buffer of `bytes` with 16-byte loads that bypass L1: *gb_per_s = bytes read
+ *                       from L2 (all SMs together) / time.  bytes <= L2 size measures L2 -> SM bandwidth, larger
+ *                       buffers fall to HBM.
+ *   amh_probe_gather    8-byte gathers at pseudo-random entries of a table of `bytes` (a power of two is used):
+ *                       *gathers_per_s.  This is the ceiling of the near-pair table look-ups of the global phase
+ *                       (one L1 wavefront per lane: about one gather per clock and SM whatever the table size in L2). */
+amh_status amh_probe_l2_read(long long bytes, int reps, double *gb_per_s, void *cuda_stream);
+amh_status amh_probe_gather(long long bytes, int reps, double *gathers_per_s, void *cuda_stream);
+
+/* Which variant of the sweep kernel amh_run would launch for a batch of B rows and this window (for reports):
+ * spec_global 1 = one warp per global proposal, ring 1 = shared-memory table ring on, cb64 1 = fp64 C-betas kept in
+ * shared memory, nspec = local proposals per pass, lanes = lanes per local proposal.  Any pointer may be NULL.  Host. */
+amh_status amh_launch_variant(amh_ctx *ctx, long long B, int window, int *spec_global, int *ring, int *cb64, int *nspec, int *lanes);
+
 const char *amh_last_error(void);
 const char *amh_version(void);
 

@@ -17,7 +17,7 @@ import numpy as np
 
 from . import build as _build
 
-__all__ = ["AMH", "AMHError", "Options", "lib", "lib_path", "default_options", "philox4x32_10",
+__all__ = ["AMH", "AMHError", "Options", "lib", "lib_path", "default_options", "philox4x32_10", "probe_l2_read", "probe_gather",
            "PROP_UNIFORM", "PROP_GRID", "PROP_GAUSSIAN", "EXPORTS"]
 
 PROP_UNIFORM, PROP_GRID, PROP_GAUSSIAN = 0, 1, 2
@@ -25,7 +25,7 @@ PROP_UNIFORM, PROP_GRID, PROP_GAUSSIAN = 0, 1, 2
 # every symbol include/amh.h declares
 EXPORTS = ["amh_default_options", "amh_default_launch_options", "amh_set_launch_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
            "amh_create_tr5", "amh_pair_geometry", "amh_run", "amh_run_host", "amh_run_pt", "amh_exchange", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
-           "amh_last_error", "amh_version"]
+           "amh_probe_l2_read", "amh_probe_gather", "amh_launch_variant", "amh_last_error", "amh_version"]
 
 
 class AMHError(RuntimeError):
@@ -129,6 +129,9 @@ def lib():
                                  C.c_void_p, C.c_void_p]
         L.amh_launch_info.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
         L.amh_launch_shape.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
+        L.amh_probe_l2_read.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_double), C.c_void_p]
+        L.amh_probe_gather.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_double), C.c_void_p]
+        L.amh_launch_variant.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 5
         L.amh_philox_test.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]
         L.amh_default_options.argtypes = [C.POINTER(_ModelOptions)]
         L.amh_default_launch_options.argtypes = [C.POINTER(_LaunchOptions)]
@@ -171,6 +174,20 @@ def _dev(t, dtype, name):
     if t.dtype != dtype or not t.is_cuda or not t.is_contiguous():
         t = t.to(device="cuda", dtype=dtype).contiguous()
     return t
+
+
+def probe_l2_read(n_bytes: int, reps: int = 20) -> float:
+    """amh_probe_l2_read: GB/s of a read-only sweep of an n_bytes buffer by every SM (L1 bypassed)."""
+    v = C.c_double()
+    _check(lib().amh_probe_l2_read(int(n_bytes), int(reps), C.byref(v), _stream_ptr()))
+    return v.value
+
+
+def probe_gather(n_bytes: int, reps: int = 5) -> float:
+    """amh_probe_gather: 8-byte gathers per second at random entries of an n_bytes table."""
+    v = C.c_double()
+    _check(lib().amh_probe_gather(int(n_bytes), int(reps), C.byref(v), _stream_ptr()))
+    return v.value
 
 
 def philox4x32_10(ctr, key):
@@ -282,8 +299,11 @@ class AMH:
         _check(lib().amh_launch_info(self._h, int(B), int(window), *[C.byref(x) for x in v]))
         u = [C.c_int() for _ in range(4)]
         _check(lib().amh_launch_shape(self._h, int(B), int(window), *[C.byref(x) for x in u]))
+        w = [C.c_int() for _ in range(5)]
+        _check(lib().amh_launch_variant(self._h, int(B), int(window), *[C.byref(x) for x in w]))
         return dict(threads_per_chain=v[0].value, smem_bytes=v[1].value, ctas_per_sm=v[2].value, n_sm=v[3].value,
-                    chains_per_cta=u[0].value, warps_per_chain=u[1].value, ring_cols=u[2].value, ring_rows=u[3].value)
+                    chains_per_cta=u[0].value, warps_per_chain=u[1].value, ring_cols=u[2].value, ring_rows=u[3].value,
+                    spec_global=w[0].value, ring=w[1].value, cb64=w[2].value, nspec=w[3].value, lanes_per_step=w[4].value)
 
     # ---- amh_run ---------------------------------------------------------------------------------
     @staticmethod

@@ -845,6 +845,97 @@ amh_status amh_run_pt(amh_ctx *c, float *states, long long B, long long n_cycles
     return AMH_OK;
 }
 
+amh_status amh_launch_variant(amh_ctx *c, long long B, int window, int *spec_global, int *ring, int *cb64, int *nspec, int *lanes)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_launch_variant: ctx is NULL");
+    if (c->param == AMH_PARAM_TR5) {
+        if (spec_global) *spec_global = 0;
+        if (ring) *ring = 0;
+        if (cb64) *cb64 = 1;
+        if (nspec) *nspec = 1;
+        if (lanes) *lanes = 128;
+        return AMH_OK;
+    }
+    const SweepShape sh = choose_shape(c, std::max<long long>(B, 1), window);
+    const long long ctas = (std::max<long long>(B, 1) + sh.C - 1) / sh.C;
+    if (spec_global) *spec_global = (c->lopt.spec_global >= 0 ? c->lopt.spec_global != 0 : (sh.W <= 2 || 2 * ctas <= c->n_sm)) ? 1 : 0;
+    if (ring) *ring = sh.R > 0 ? 1 : 0;
+    if (cb64) *cb64 = sh.cb64;
+    if (nspec) *nspec = sh.nspec;
+    if (lanes) *lanes = sh.gl;
+    return AMH_OK;
+}
+
+static amh_status probe_common(long long bytes, int reps, void **buf, cudaStream_t st)
+{
+    if (bytes < (1 << 20) || reps < 1) return fail(AMH_ERR_INVALID_ARG, "amh_probe: bytes >= 1 MiB and reps >= 1 are required");
+    AMH_CUDA(cudaMalloc(buf, (size_t)bytes));
+    cudaError_t e = cudaMemsetAsync(*buf, 0, (size_t)bytes, st);
+    if (e != cudaSuccess) { cudaFree(*buf); return fail(AMH_ERR_CUDA, "amh_probe: %s", cudaGetErrorString(e)); }
+    return AMH_OK;
+}
+
+amh_status amh_probe_l2_read(long long bytes, int reps, double *gb_per_s, void *cuda_stream)
+{
+    if (!gb_per_s) return fail(AMH_ERR_INVALID_ARG, "amh_probe_l2_read: output is NULL");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    void *buf = nullptr;
+    amh_status stt = probe_common(bytes, reps, &buf, st);
+    if (stt != AMH_OK) return stt;
+    int dev = 0, n_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    unsigned *out = reinterpret_cast<unsigned *>(buf);
+    const size_t n16 = (size_t)bytes / 16;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    amh::l2_read_kernel<<<n_sm * 2, 512, 0, st>>>(reinterpret_cast<const uint4 *>(buf), n16, 1, out);
+    cudaEventRecord(e0, st);
+    amh::l2_read_kernel<<<n_sm * 2, 512, 0, st>>>(reinterpret_cast<const uint4 *>(buf), n16, reps, out);
+    cudaEventRecord(e1, st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.0f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (e != cudaSuccess) return fail(AMH_ERR_CUDA, "amh_probe_l2_read: %s", cudaGetErrorString(e));
+    // every CTA reads the whole buffer `reps` times (rounded up to its 4 x blockDim chunks)
+    const double chunks = std::ceil((double)n16 / (512.0 * 4.0));
+    *gb_per_s = (double)n_sm * 2.0 * reps * chunks * 512.0 * 4.0 * 16.0 / (ms * 1e-3) / 1e9;
+    return AMH_OK;
+}
+
+amh_status amh_probe_gather(long long bytes, int reps, double *gathers_per_s, void *cuda_stream)
+{
+    if (!gathers_per_s) return fail(AMH_ERR_INVALID_ARG, "amh_probe_gather: output is NULL");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    size_t n8 = 1;
+    while (n8 * 2 * 8 <= (size_t)bytes) n8 *= 2;
+    void *buf = nullptr;
+    amh_status stt = probe_common((long long)(n8 * 8), reps, &buf, st);
+    if (stt != AMH_OK) return stt;
+    int dev = 0, n_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    float *out = reinterpret_cast<float *>(buf);
+    const int iters = 200;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    amh::gather_kernel<<<n_sm * 4, 256, 0, st>>>(reinterpret_cast<const float2 *>(buf), (unsigned)(n8 - 1), iters, out);
+    cudaEventRecord(e0, st);
+    for (int r = 0; r < reps; ++r)
+        amh::gather_kernel<<<n_sm * 4, 256, 0, st>>>(reinterpret_cast<const float2 *>(buf), (unsigned)(n8 - 1), iters, out);
+    cudaEventRecord(e1, st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.0f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (e != cudaSuccess) return fail(AMH_ERR_CUDA, "amh_probe_gather: %s", cudaGetErrorString(e));
+    *gathers_per_s = (double)n_sm * 4.0 * 256.0 * iters * 8.0 * reps / (ms * 1e-3);
+    return AMH_OK;
+}
+
 amh_status amh_philox_test(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long count, void *cuda_stream)
 {
     if (count < 0 || (count > 0 && (!ctr || !key || !out))) return fail(AMH_ERR_INVALID_ARG, "amh_philox_test: bad arguments");

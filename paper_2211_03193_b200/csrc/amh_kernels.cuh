@@ -162,6 +162,50 @@ __global__ void exchange_kernel(const float *__restrict__ V, float *__restrict__
     if (n_accepted && ok) atomicAdd(n_accepted, 1ull);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Measurement hooks: the two memory ceilings of the pair loops, measured on the device the
+// library runs on.  Neither is on the hot path.
+//   l2_read_kernel    read-only sweep of a buffer with 16-byte loads that bypass L1 (ld.global.cg): every SM reads the
+//                     WHOLE buffer, so a buffer that fits in L2 is served by L2 after the first touch
+//   gather_kernel     8-byte gathers at pseudo-random entries of a table (the access pattern of a near pair's lerp
+//                     operands): bounded by one L1 wavefront per lane and clock, not by L2 bandwidth
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(512) l2_read_kernel(const uint4 *__restrict__ p, size_t n16, int reps, unsigned *__restrict__ out)
+{
+    unsigned acc = 0;
+    // CTA b starts at its own offset so that the SMs do not walk the buffer in lockstep
+    const size_t start = ((size_t)blockIdx.x * 7919u * blockDim.x) % n16;
+    for (int r = 0; r < reps; ++r) {
+        for (size_t q0 = 0; q0 < n16; q0 += (size_t)blockDim.x * 4) {
+            uint4 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                size_t q = start + q0 + (size_t)u * blockDim.x + threadIdx.x;
+                if (q >= n16) q -= n16;
+                if (q >= n16) q %= n16;
+                v[u] = __ldcg(p + q);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) acc += v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
+        }
+    }
+    if (acc == 0x9e3779b9u) out[0] = acc;                  // keeps the loads alive
+}
+
+__global__ void __launch_bounds__(256) gather_kernel(const float2 *__restrict__ p, unsigned mask, int iters, float *__restrict__ out)
+{
+    float acc = 0.0f;
+    unsigned idx = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 12345u;
+    for (int it = 0; it < iters; ++it) {
+        float2 v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { idx = idx * 1664525u + 1013904223u; v[q] = __ldg(p + ((idx >> 4) & mask)); }
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc += v[q].x + v[q].y;
+    }
+    if (acc == 1234.5f) out[0] = acc;
+}
+
 // the running minimum of the sweep-end energies over the cycles of amh_run_pt
 __global__ void min_into_kernel(float *__restrict__ dst, const float *__restrict__ src, long long count, int first)
 {

@@ -48,7 +48,13 @@ def test_default_options_and_argument_checks_without_a_device():
     p = np.full((2, 2, 64), 1 / 64, np.float32)
     assert lib.amh_create(C.byref(h), 0, 0, p.ctypes.data, edges.ctypes.data, 64, None, None) == 1   # n_res < 1
     assert b"n_res" in lib.amh_last_error()
-    assert lib.amh_create(C.byref(h), 2, 1, p.ctypes.data, edges.ctypes.data, 64, None, None) == 2   # TR5 unsupported
+    assert lib.amh_create(C.byref(h), 2, 1, p.ctypes.data, edges.ctypes.data, 64, None, None) == 1   # TR5: amh_create_tr5 builds those
+    assert b"amh_create_tr5" in lib.amh_last_error()
+    assert lib.amh_create_tr5(C.byref(h), 2, p.ctypes.data, edges.ctypes.data, 64, None, None, None) == 1   # maps missing
+    lo = pkg.default_options(warps_per_chain=99)
+    assert lib.amh_set_launch_options(None, C.byref(lo.launch)) == 1
+    v = C.c_double()
+    assert lib.amh_probe_l2_read(16, 1, C.byref(v), None) == 1                                     # < 1 MiB
     assert lib.amh_create(C.byref(h), 2, 0, None, edges.ctypes.data, 64, None, None) == 1
     assert lib.amh_create(C.byref(h), 2, 0, p.ctypes.data, edges.ctypes.data, 1, None, None) == 1
     assert lib.amh_destroy(None) == 0

@@ -69,3 +69,26 @@ def test_chain_sharding_world_size_2_gloo():
     for p in procs:
         p.join(timeout=30)
     assert res == {0: "ok", 1: "ok"}, res
+
+
+@pytest.mark.timeout(300)
+def test_bench_gpus_2_starts_two_ranks_itself():
+    # `bench.py --gpus 2` WITHOUT a launcher environment must start the two ranks itself (torch.distributed.run on 127.0.0.1)
+    # and report n_gpus = the ranks that ran; --dry-run takes the same launcher and sharding path with gloo and no kernels
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-run", "--config", "0"],
+                         capture_output=True, text=True, env=env, timeout=280)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads([x for x in out.stdout.splitlines() if x.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["dry_run"] is True
+    B = 32
+    assert [r[:3] for r in line["shards"]] == [[0, 0, B], [1, B, 2 * B]]
+    assert line["shards"][0][3] != line["shards"][1][3]                       # the ranks hold different chains
+    assert line["config"]["parallelism"] == "chains sharded x2"
+    # one rank: no launcher, n_gpus 1
+    out1 = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "1", "--dry-run", "--config", "0"],
+                          capture_output=True, text=True, env=env, timeout=120)
+    l1 = json.loads([x for x in out1.stdout.splitlines() if x.startswith("{")][-1])
+    assert l1["n_gpus"] == 1 and l1["shards"] == [line["shards"][0]]
