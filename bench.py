@@ -407,6 +407,7 @@ def main():
     ap.add_argument("--ring-cols", type=int, default=0)
     ap.add_argument("--lanes-per-step", type=int, default=0)
     ap.add_argument("--spec-global", type=int, default=-1)
+    ap.add_argument("--local-stride", type=int, default=0, help="NEXT-4 variant: strided order of the local sweeps (experiments only; the line says so; not Alg. 1's trajectories)")
     ap.add_argument("--exchange", action="store_true", help="configs with temperature replicas: amh_run_pt (replica exchange after every cycle, NEXT-3) instead of amh_run; the line says so")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -421,7 +422,7 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     cfg = gi.CONFIGS[args.config]
-    overridden = bool(args.sweeps or args.chains)
+    overridden = bool(args.sweeps or args.chains or args.local_stride)
     if overridden:
         import dataclasses
         cfg = dataclasses.replace(cfg, n_sweeps=args.sweeps or cfg.n_sweeps, B=args.chains or cfg.B)
@@ -491,6 +492,9 @@ def main():
     launch_over = dict(warps_per_chain=args.warps_per_chain, chains_per_cta=args.chains_per_cta, spec_local=args.spec_local,
                        ring_cols=args.ring_cols, lanes_per_step=args.lanes_per_step, spec_global=args.spec_global)
     wl = Workload(pkg, torch, cfg, rank, world, launch_over)
+    if args.local_stride:
+        wl.kw["local_stride"] = args.local_stride
+        workload["order"] = "NEXT-4 variant: strided local sweeps, stride %d (not Alg. 1's order)" % args.local_stride
     g, kw, states, B, n = wl.g, wl.kw, wl.states, cfg.B, cfg.n
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
     stream = torch.cuda.current_stream()

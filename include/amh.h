@@ -93,6 +93,11 @@ typedef struct {
     int n_local;        /* sweeps per cycle judged on V_local      (>= 0; n_global + n_local >= 1) */
     int window;         /* radius w in residues, inclusive, clamped at the chain ends (>= 0) */
     int global_first;   /* 1 = Alg. 1 order (global sweeps first in each cycle); 0 = local first */
+    int local_stride;   /* NEXT-4 (a VARIANT of Alg. 1; R26): 0 = the paper's order k = 0..n-1.
+                           s >= 1: local sweeps visit the residues in colour classes o = 0..s-1 (c = o, o+s, o+2s, ...), phi_c
+                           then psi_c; with s >= 2 * window + 1 the windows of a class do not overlap, their proposals do not
+                           interact, and the kernel evaluates a class in parallel with nothing speculative.  The draws stay
+                           keyed by (sweep, variable).  Global sweeps keep k = 0..n-1.  AMH_PARAM_PHI_PSI only. */
 } amh_schedule;
 
 /* R13.  T_t = t_start * (t_end/t_start)^(t/(ramp_sweeps-1)) for absolute sweep index t, constant

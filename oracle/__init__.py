@@ -52,7 +52,7 @@ class _RunParams(C.Structure):
                 ("prop_mode", C.c_int), ("grid", C.c_int),
                 ("sigma_start", C.c_double), ("sigma_end", C.c_double), ("ramp_sigma", C.c_longlong),
                 ("seed", C.c_ulonglong), ("chain_offset", C.c_longlong),
-                ("only_k", C.c_int), ("trace_steps", C.c_int), ("n_threads", C.c_int), ("pad_", C.c_int)]
+                ("only_k", C.c_int), ("trace_steps", C.c_int), ("n_threads", C.c_int), ("local_stride", C.c_int)]
 
 
 class _Outputs(C.Structure):
@@ -93,6 +93,12 @@ def philox4x32_10(ctr, key) -> np.ndarray:
     out = np.zeros(4, dtype=np.uint32)
     lib().amho_philox4x32_10(_p(c), _p(k), _p(out))
     return out
+
+
+def sweep_order(n_res: int, is_global: bool, stride: int) -> np.ndarray:
+    """The variables in the order a sweep visits them (NEXT-4): Alg. 1's 0..n-1, or the strided order of a local sweep."""
+    return np.array([lib().amho_sweep_order(C.c_int(p), C.c_int(int(is_global)), C.c_int(n_res), C.c_int(stride))
+                     for p in range(2 * n_res)], dtype=np.int64)
 
 
 def default_geom(**over) -> Geom:
@@ -158,24 +164,24 @@ class Model:
     # -- Alg. 1 ---------------------------------------------------------------------------------
     def _params(self, n_sweeps, sweep_offset, n_global, n_local, window, global_first, t_start, t_end,
                 ramp_sweeps, per_chain_T, prop_mode, grid, sigma_start, sigma_end, ramp_sigma, seed,
-                chain_offset, only_k, trace_steps, n_threads):
+                chain_offset, only_k, trace_steps, n_threads, local_stride=0):
         return _RunParams(n_sweeps, sweep_offset, n_global, n_local, window, int(global_first),
                           t_start, t_end, ramp_sweeps,
                           None if per_chain_T is None else per_chain_T.ctypes.data,
                           prop_mode, grid, sigma_start, sigma_end, ramp_sigma, seed, chain_offset,
-                          only_k, trace_steps, n_threads, 0)
+                          only_k, trace_steps, n_threads, local_stride)
 
     def run(self, states, n_sweeps, *, n_global=1, n_local=10, window=8, global_first=True,
             t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
             sigma_start=0.0, sigma_end=0.0, ramp_sigma=0, seed=1, chain_offset=0, sweep_offset=0,
-            only_k=-1, trace_steps=0, n_threads=0, record_sweeps=False):
+            only_k=-1, trace_steps=0, n_threads=0, record_sweeps=False, local_stride=0):
         """Free-running AMH; returns a dict (states are returned, the input is not modified)."""
         s = np.array(states, dtype=np.float32, order="C").reshape(-1, self.n)
         B = s.shape[0]
         pct = None if per_chain_T is None else np.ascontiguousarray(per_chain_T, dtype=np.float32)
         prm = self._params(n_sweeps, sweep_offset, n_global, n_local, window, global_first, t_start, t_end,
                            ramp_sweeps, pct, prop_mode, grid, sigma_start, sigma_end, ramp_sigma, seed,
-                           chain_offset, only_k, trace_steps, n_threads)
+                           chain_offset, only_k, trace_steps, n_threads, local_stride)
         r = dict(
             energy=np.zeros(B), best_energy=np.zeros(B), best_state=np.zeros((B, self.n), np.float32),
             n_accept_local=np.zeros(B, np.int64), n_accept_global=np.zeros(B, np.int64),
@@ -195,7 +201,7 @@ class Model:
     def follow(self, states, steps, forced_acc, *, n_global=1, n_local=10, window=8, global_first=True,
                t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
                sigma_start=0.0, sigma_end=0.0, ramp_sigma=0, seed=1, chain_offset=0, sweep_offset=0,
-               n_threads=0, forced_prop=None):
+               n_threads=0, forced_prop=None, local_stride=0):
         """Follow mode: replay `steps` proposals taking the decisions in forced_acc [B][steps]; with
         forced_prop [B][steps] also the proposed values (Gaussian mode, R5) - "prop" in the result
         is still this implementation's own proposal."""
@@ -205,7 +211,7 @@ class Model:
         pct = None if per_chain_T is None else np.ascontiguousarray(per_chain_T, dtype=np.float32)
         prm = self._params(0, sweep_offset, n_global, n_local, window, global_first, t_start, t_end,
                            ramp_sweeps, pct, prop_mode, grid, sigma_start, sigma_end, ramp_sigma, seed,
-                           chain_offset, -1, 0, n_threads)
+                           chain_offset, -1, 0, n_threads, local_stride)
         prop = np.zeros((B, steps), np.float32)
         dE = np.zeros((B, steps))
         g = np.zeros((B, steps))

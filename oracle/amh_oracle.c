@@ -245,7 +245,7 @@ typedef struct {
     int only_k;                           /* test hook (pin P5 iii): propose only this variable; -1 = all */
     int trace_steps;                      /* first trace_steps proposals of the call are traced */
     int n_threads;                        /* OpenMP threads over chains; <= 0 = default */
-    int pad_;
+    int local_stride;                     /* NEXT-4: 0 = Alg. 1's order k = 0..n-1; s > 0 = the strided order of local sweeps */
 } amho_run_params;
 
 typedef struct {                          /* every pointer optional */
@@ -281,6 +281,24 @@ static double sigma_at(const amho_run_params *p, long long t)
     if (p->sigma_start == p->sigma_end || p->ramp_sigma <= 1 || t <= 0) return p->sigma_start;
     if (t >= p->ramp_sigma - 1) return p->sigma_end;
     return p->sigma_start + (p->sigma_end - p->sigma_start) * ((double)t / (double)(p->ramp_sigma - 1));
+}
+
+/* NEXT-4 (PAPER.md:105, 114 give the order being changed): the variable visited at position p of a sweep.
+ * Alg. 1 (stride <= 0, and every global sweep): k = p.  Strided local sweep with stride s: the residues are visited in
+ * colour classes o = 0 .. s-1 (c = o, o + s, o + 2s, ...), both variables of a residue in turn (phi_c, then psi_c).  With
+ * s >= 2w + 1 the windows of the residues of one class do not overlap, so their proposals do not interact: an accepted
+ * move turns everything right of it rigidly and leaves every other window's internal distances unchanged (R26). */
+int amho_sweep_order(int p, int is_global, int L, int stride)
+{
+    if (is_global || stride <= 0) return p;
+    int r = p / 2;
+    const int par = p % 2;
+    for (int o = 0; o < stride && o < L; ++o) {
+        const int cnt = (L - o + stride - 1) / stride;
+        if (r < cnt) return 2 * (o + r * stride) + par;
+        r -= cnt;
+    }
+    return p;
 }
 
 /* R5: the proposed value for variable k.  UNIFORM and GRID are a single IEEE fp32 operation chain
@@ -353,7 +371,8 @@ int amho_run(const amho_model *m, const amho_run_params *p, float *states, long 
             for (long long t = p->sweep_offset; t < p->sweep_offset + p->n_sweeps; ++t) {
                 const int is_global = phase_is_global(p, t);
                 const double T = amho_temperature(p, t, row);
-                for (int k = 0; k < n; ++k) {
+                for (int pos = 0; pos < n; ++pos) {
+                    const int k = amho_sweep_order(pos, is_global, L, p->local_stride);
                     if (p->only_k >= 0 && k != p->only_k) continue;
                     const uint64_t step = (uint64_t)t * (uint64_t)n + (uint64_t)k;
                     const float s_new = propose(p, chain, step, t, s[k]);
@@ -418,10 +437,11 @@ int amho_follow(const amho_model *m, const amho_run_params *p, float *states, lo
             float *s = states + row * n;
             const uint64_t chain = (uint64_t)(p->chain_offset + row);
             for (int q = 0; q < steps; ++q) {
-                const uint64_t step = (uint64_t)p->sweep_offset * (uint64_t)n + (uint64_t)q;
-                const long long t = (long long)(step / (uint64_t)n);
-                const int k = (int)(step % (uint64_t)n);
+                const uint64_t at = (uint64_t)p->sweep_offset * (uint64_t)n + (uint64_t)q;
+                const long long t = (long long)(at / (uint64_t)n);
                 const int is_global = phase_is_global(p, t);
+                const int k = amho_sweep_order((int)(at % (uint64_t)n), is_global, L, p->local_stride);
+                const uint64_t step = (uint64_t)t * (uint64_t)n + (uint64_t)k;      /* the draws are keyed by the variable */
                 const double T = amho_temperature(p, t, row);
                 size_t z = (size_t)row * steps + q;
                 const float s_own = propose(p, chain, step, t, s[k]);

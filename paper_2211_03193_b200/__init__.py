@@ -71,7 +71,7 @@ class _OrientationMaps(C.Structure):       # amh_orientation_maps
 
 
 class _Schedule(C.Structure):
-    _fields_ = [("n_global", C.c_int), ("n_local", C.c_int), ("window", C.c_int), ("global_first", C.c_int)]
+    _fields_ = [("n_global", C.c_int), ("n_local", C.c_int), ("window", C.c_int), ("global_first", C.c_int), ("local_stride", C.c_int)]
 
 
 class _Temperature(C.Structure):
@@ -308,15 +308,15 @@ class AMH:
     # ---- amh_run ---------------------------------------------------------------------------------
     @staticmethod
     def _structs(n_global, n_local, window, global_first, t_start, t_end, ramp_sweeps, per_chain_T_ptr,
-                 prop_mode, grid, sigma_start=0.0, sigma_end=0.0, ramp_sigma=0):
-        return (_Schedule(n_global, n_local, window, int(bool(global_first))),
+                 prop_mode, grid, sigma_start=0.0, sigma_end=0.0, ramp_sigma=0, local_stride=0):
+        return (_Schedule(n_global, n_local, window, int(bool(global_first)), int(local_stride)),
                 _Temperature(t_start, t_end, ramp_sweeps, per_chain_T_ptr),
                 _Proposal(prop_mode, grid, sigma_start, sigma_end, ramp_sigma))
 
     def run(self, states, n_sweeps: int, *, n_global=1, n_local=10, window=8, global_first=True,
             t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
             sigma_start=0.0, sigma_end=0.0, ramp_sigma=0,
-            seed=1, chain_offset=0, sweep_offset=0, trace_steps=0, energy_threshold=None,
+            seed=1, chain_offset=0, sweep_offset=0, trace_steps=0, energy_threshold=None, local_stride=0,
             want=("energy", "best_energy", "best_state", "n_accept_local", "n_accept_global"), stream=None):
         """amh_run on a DEVICE batch; `states` (torch.float32 [B][n], cuda) is updated in place.
         Returns a dict of device tensors for the outputs named in `want` (+ traces, first_hit_sweep)."""
@@ -353,7 +353,7 @@ class AMH:
                 raise ValueError("per_chain_T must have B entries")
         sc, tp, pr = self._structs(n_global, n_local, window, global_first, t_start, t_end, ramp_sweeps,
                                    pct.data_ptr() if pct is not None else None, prop_mode, grid,
-                                   sigma_start, sigma_end, ramp_sigma)
+                                   sigma_start, sigma_end, ramp_sigma, local_stride)
         _check(lib().amh_run(self._h, s.data_ptr(), B, int(n_sweeps), int(sweep_offset), int(chain_offset),
                              C.byref(sc), C.byref(tp), C.byref(pr), int(seed), C.byref(o), _stream_ptr(stream)))
         r["_keepalive"] = pct
@@ -397,7 +397,7 @@ class AMH:
     def run_host(self, states: np.ndarray, n_sweeps: int, *, n_global=1, n_local=10, window=8, global_first=True,
                  t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,
                  sigma_start=0.0, sigma_end=0.0, ramp_sigma=0,
-                 seed=1, chain_offset=0, sweep_offset=0, trace_steps=0, energy_threshold=None,
+                 seed=1, chain_offset=0, sweep_offset=0, trace_steps=0, energy_threshold=None, local_stride=0,
                  want=("energy", "best_energy")):
         """amh_run_host: HOST numpy buffers in and out (states updated in place); synchronous."""
         if not (isinstance(states, np.ndarray) and states.dtype == np.float32 and states.flags.c_contiguous):
@@ -428,7 +428,7 @@ class AMH:
             pct = np.ascontiguousarray(per_chain_T, dtype=np.float32)
         sc, tp, pr = self._structs(n_global, n_local, window, global_first, t_start, t_end, ramp_sweeps,
                                    pct.ctypes.data if pct is not None else None, prop_mode, grid,
-                                   sigma_start, sigma_end, ramp_sigma)
+                                   sigma_start, sigma_end, ramp_sigma, local_stride)
         _check(lib().amh_run_host(self._h, s.ctypes.data, B, int(n_sweeps), int(sweep_offset), int(chain_offset),
                                   C.byref(sc), C.byref(tp), C.byref(pr), int(seed), C.byref(o), _stream_ptr()))
         return r

@@ -284,6 +284,9 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
     AMH_SMEM_ATTR(false, false, false); AMH_SMEM_ATTR(false, false, true); AMH_SMEM_ATTR(false, true, false); AMH_SMEM_ATTR(false, true, true);
     AMH_SMEM_ATTR(true, false, false); AMH_SMEM_ATTR(true, false, true); AMH_SMEM_ATTR(true, true, false); AMH_SMEM_ATTR(true, true, true);
 #undef AMH_SMEM_ATTR
+#define AMH_SMEM_ATTR_S(SG_, CB_) AMH_CUDA_C(cudaFuncSetAttribute(amh::sweep_kernel<SG_, false, CB_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem))
+    AMH_SMEM_ATTR_S(false, false); AMH_SMEM_ATTR_S(false, true); AMH_SMEM_ATTR_S(true, false); AMH_SMEM_ATTR_S(true, true);
+#undef AMH_SMEM_ATTR_S
     AMH_CUDA_C(cudaFuncSetAttribute(amh::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->max_smem));
 #undef AMH_CUDA_C
     *out = c;
@@ -492,7 +495,7 @@ amh_status amh_coords(amh_ctx *c, const float *states, long long B, float *cb_ou
 // per pass, lanes per local proposal.
 struct SweepShape { int C, W, R, ring_rows, cb64, nspec, gl, wpts; size_t smem; };
 
-static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
+static SweepShape choose_shape(const amh_ctx *c, long long B, int window, int strided = 0)
 {
     const int L = c->m.L;
     const int w_eff = std::min(window, std::max(L - 1, 0));
@@ -509,7 +512,7 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
         return std::max(1, ns);
     };
     auto ring_for = [&](int C, int ns) -> int {               // slots: the window's columns + reach of a pass + drift between teams
-        if (c->lopt.ring_cols < 0 || sh.ring_rows == 0 || span > c->band_dmax || c->m.min_sep > amh::kRingPadRows + 1) return 0;
+        if (strided || c->lopt.ring_cols < 0 || sh.ring_rows == 0 || span > c->band_dmax || c->m.min_sep > amh::kRingPadRows + 1) return 0;
         if (c->lopt.ring_cols > 0) return std::max(c->lopt.ring_cols, w_eff + 3);
         return w_eff + 3 + (ns + 1) / 2 + (C > 1 ? 4 : 0);
     };
@@ -518,7 +521,8 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
         const int W = c->lopt.warps_per_chain;
         return W > 0 ? std::max(1, std::min(W, amh::kMaxTeamWarps / C_)) : std::max(1, std::min(amh::kMaxTeamWarps / C_, 8));
     };
-    auto fits = [&](int C, int R, int ns) { return amh::sweep_smem_bytes(L, C, warps_for(C), R, sh.ring_rows, c->m.row_stride, sh.cb64, ns, sh.wpts) <= budget; };
+    const int cbn_f = strided ? 2 : 1;                       // strided sweeps keep two sets of columns per proposal
+    auto fits = [&](int C, int R, int ns) { return amh::sweep_smem_bytes(L, C, warps_for(C), R, sh.ring_rows, c->m.row_stride, sh.cb64, cbn_f * ns, sh.wpts) <= budget; };
     // chains per CTA: spread the batch over the SMs (one CTA each) and keep as many teams resident as shared memory
     // allows; the ring is added only when it fits beside them (warps in flight are worth more than the ring)
     int C = c->lopt.chains_per_cta;
@@ -546,7 +550,7 @@ static SweepShape choose_shape(const amh_ctx *c, long long B, int window)
     if (R > 0) ns = std::max(1, std::min(ns, 2 * (R - w_eff - 2) - 1));
     sh.C = C; sh.W = W; sh.R = R; sh.nspec = ns;
     if (R == 0) sh.ring_rows = 0;
-    sh.smem = amh::sweep_smem_bytes(L, C, W, R, sh.ring_rows, c->m.row_stride, sh.cb64, ns, sh.wpts);
+    sh.smem = amh::sweep_smem_bytes(L, C, W, R, sh.ring_rows, c->m.row_stride, sh.cb64, cbn_f * ns, sh.wpts);
     return sh;
 }
 
@@ -607,6 +611,9 @@ static amh_status check_run(const amh_ctx *c, const float *states, long long B, 
     if (sc->n_global < 0 || sc->n_local < 0 || sc->n_global + sc->n_local < 1)
         return fail(AMH_ERR_INVALID_ARG, "amh_run: schedule needs n_global, n_local >= 0 and n_global + n_local >= 1");
     if (sc->window < 0) return fail(AMH_ERR_INVALID_ARG, "amh_run: window = %d < 0", sc->window);
+    if (sc->local_stride < 0) return fail(AMH_ERR_INVALID_ARG, "amh_run: local_stride = %d < 0", sc->local_stride);
+    if (sc->local_stride > 0 && c->param == AMH_PARAM_TR5)
+        return fail(AMH_ERR_UNSUPPORTED, "amh_run: the strided sweep order is built for AMH_PARAM_PHI_PSI only");
     if (!tp->per_chain_T && !(tp->t_start > 0.0 && tp->t_end > 0.0 && std::isfinite(tp->t_start) && std::isfinite(tp->t_end)))
         return fail(AMH_ERR_INVALID_ARG, "amh_run: temperatures must be finite and > 0");
     if (pr) {
@@ -631,6 +638,7 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     std::memset(&a, 0, sizeof a);
     a.states = states; a.B = B; a.n_sweeps = n_sweeps; a.sweep_offset = sweep_offset; a.chain_offset = chain_offset;
     a.n_global = sc->n_global; a.n_local = sc->n_local; a.window = sc->window; a.global_first = sc->global_first ? 1 : 0;
+    a.local_stride = sc->local_stride;
     a.t_start = tp->t_start; a.t_end = tp->t_end; a.ramp_sweeps = tp->ramp_sweeps; a.per_chain_T = tp->per_chain_T;
     a.prop_mode = pr ? pr->mode : AMH_PROP_UNIFORM; a.grid = pr ? pr->grid : 0;
     a.sigma_start = pr ? pr->sigma_start : 0.0; a.sigma_end = pr ? pr->sigma_end : 0.0; a.ramp_sigma = pr ? pr->ramp_sweeps : 0;
@@ -660,7 +668,7 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
         AMH_CUDA(cudaGetLastError());
         return AMH_OK;
     }
-    const SweepShape sh = choose_shape(c, B, sc->window);
+    const SweepShape sh = choose_shape(c, B, sc->window, sc->local_stride > 0);
     if (sh.smem > (size_t)c->max_smem)
         return fail(AMH_ERR_UNSUPPORTED, "amh_run: L = %d, window = %d, %d chains x %d warps need %zu B of shared memory, device allows %d",
                     c->m.L, sc->window, sh.C, sh.W, sh.smem, c->max_smem);
@@ -673,6 +681,18 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     const bool sg = c->lopt.spec_global >= 0 ? c->lopt.spec_global != 0 : (sh.W <= 2 || 2 * ctas <= c->n_sm);
     const unsigned threads = 32 * (sh.C * sh.W + 1);
     const int variant = (sg ? 4 : 0) | (sh.R > 0 ? 2 : 0) | (sh.cb64 ? 1 : 0);
+    if (sc->local_stride > 0) {                              // NEXT-4's own instantiations (no ring)
+#define AMH_LAUNCH_S(SG_, CB_) amh::sweep_kernel<SG_, false, CB_, true><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a)
+        switch (variant & 5) {
+        case 0: AMH_LAUNCH_S(false, false); break;
+        case 1: AMH_LAUNCH_S(false, true); break;
+        case 4: AMH_LAUNCH_S(true, false); break;
+        default: AMH_LAUNCH_S(true, true); break;
+        }
+#undef AMH_LAUNCH_S
+        AMH_CUDA(cudaGetLastError());
+        return AMH_OK;
+    }
 #define AMH_LAUNCH(SG_, RING_, CB_) amh::sweep_kernel<SG_, RING_, CB_><<<(unsigned)ctas, threads, sh.smem, st>>>(c->m, a)
     switch (variant) {
     case 0: AMH_LAUNCH(false, false, false); break;

@@ -50,6 +50,7 @@ struct RunArgs {
     float *states;
     long long B, n_sweeps, sweep_offset, chain_offset;
     int n_global, n_local, window, global_first;
+    int local_stride;                    // NEXT-4: 0 = Alg. 1's order; s > 0 = strided order of the local sweeps
     double t_start, t_end;
     long long ramp_sweeps;
     const float *per_chain_T;
@@ -636,7 +637,8 @@ __device__ __forceinline__ double team_full_energy(const DevModel &m, const floa
 // carries the other's pair loop in its register budget)
 // RING: the local phase reads its rows from the shared-memory ring (a.ring_cols > 0) or gathers them from L2.
 // CB64: the fp64 C-betas are kept in shared memory (a.cb64) or rebuilt from N, CA, C.
-template <bool SG, bool RING, bool CB64>
+// STRIDED: the local sweeps take NEXT-4's strided order (its own instantiations: Alg. 1's kernels do not carry that code).
+template <bool SG, bool RING, bool CB64, bool STRIDED = false>
 __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, RunArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -699,7 +701,8 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     if (slot >= nvalid) return;
 
     // ================= team: one chain =====================================================================
-    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L, a.cb64, a.nspec, a.wpts, W);
+    const int cbn_rows = a.local_stride > 0 ? 2 * a.nspec : a.nspec;   // strided sweeps also keep the columns' current C-betas
+    unsigned char *cbase = smem_raw + chains_off + (size_t)slot * chain_smem_bytes(L, a.cb64, cbn_rows, a.wpts, W);
     constexpr bool cb64 = CB64;
     const int na = cb64 ? 4 : 3;                            // atoms per residue kept in fp64
     double *X = reinterpret_cast<double *>(cbase), *Y = X + na * L, *Z = Y + na * L;
@@ -708,7 +711,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     float4 *cb4 = reinterpret_cast<float4 *>(sp_T + kMaxSpec);
     float4 *blk4 = cb4 + L;
     float4 *cbn = blk4 + (L + kBlk - 1) / kBlk;
-    float *s = reinterpret_cast<float *>(cbn + (size_t)a.nspec * a.wpts);
+    float *s = reinterpret_cast<float *>(cbn + (size_t)cbn_rows * a.wpts);
     float *b_sp = s + n;
 
     const long long row = row0 + slot;
@@ -801,6 +804,184 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
             team_bar(bar_id, nthreads);
         }
         int k = 0, batch_start = 0, batch_end = 0;
+        if (STRIDED && !gp && a.local_stride > 0) {
+            // ======== NEXT-4: strided local sweep (R26) ========================================================
+            // The residues are visited in colour classes o = 0 .. s-1 (c = o, o + s, ...), phi_c then psi_c.  With
+            // s >= 2w + 1 the windows of a class do not overlap: an accepted move turns everything right of it rigidly, which
+            // changes no distance inside another window, so the proposals of a class do not interact and the order inside a
+            // class is immaterial.  A pass evaluates the same variable (phi, then psi) of up to nspec residues of a class
+            // against the current state, one group each, decides them all, and commits every accepted one together.
+            // Nothing is speculative here: every evaluation stands.  (s < 2w + 1: one proposal per pass, in the same order.)
+            const int sd = a.local_stride;
+            const bool indep = sd >= 2 * w_eff + 1;
+            float4 *cbo = cbn + (size_t)nspec * a.wpts;             // the current C-betas of the columns (the old state's sum)
+            int pos_class = 0;                                      // position of the class's first variable in the sweep
+            for (int o = 0; o < sd && o < L; ++o) {
+                const int cnt = (L - o + sd - 1) / sd;
+                const int chunk = indep ? nspec : 1;
+                for (int r0 = 0; r0 < cnt; r0 += indep ? chunk : 1) {
+                  for (int par = 0; par < 2; ++par) {
+                    // the independent order: all phi of the chunk, then all psi; the sequential one: phi_c, psi_c per residue
+                    const int S = min(chunk, cnt - r0);
+                    // ---- draws of the pass: lane r of warp 0 the proposal, of the last warp the uniform -------------
+                    if (lane < S && (warp == 0 || warp == nwarps - 1)) {
+                        const int kk = 2 * (o + (r0 + lane) * sd) + par;
+                        const unsigned long long step = (unsigned long long)t * (unsigned long long)n + (unsigned long long)kk;
+                        if (warp == 0) {
+                            uint32_t x1;
+                            const uint32_t x0 = draw01(a.seed, chain, step, PURPOSE_PROPOSAL, x1);
+                            float sp;
+                            if (a.prop_mode == 2) {
+                                const double u1 = ((double)(x0 >> 8) + 1.0) * 5.9604644775390625e-08;
+                                const double u2 = (double)(x1 >> 8) * 5.9604644775390625e-08;
+                                const double z = sqrt(-2.0 * log(u1)) * cos(6.283185307179586 * u2);
+                                double v = (double)s[kk] + sigma_t * z;
+                                v -= 6.283185307179586 * floor((v + 3.141592653589793) / 6.283185307179586);
+                                sp = (float)v;
+                                if (sp >= 3.14159274101257324f) sp -= 2.0f * 3.14159274101257324f;
+                            } else if (a.prop_mode == 1) {
+                                const int mm = (int)(x0 % (uint32_t)a.grid);
+                                sp = __fmul_rn(__fdiv_rn((float)(2 * mm - a.grid), (float)a.grid), 3.14159274101257324f);
+                            } else {
+                                const int h = (int)(x0 >> 8) - (1 << 23);
+                                sp = __fmul_rn((float)h * 1.1920928955078125e-07f, 3.14159274101257324f);
+                            }
+                            double sdl, cdl;
+                            sincos((double)sp - (double)s[kk], &sdl, &cdl);
+                            b_sp[lane] = sp; b_cd[lane] = cdl; b_sd[lane] = sdl;
+                        }
+                        if (warp == nwarps - 1) {
+                            const uint32_t x0 = draw0(a.seed, chain, step, PURPOSE_ACCEPT);
+                            b_lu[lane] = log((double)((x0 >> 8) + 1u) * 5.9604644775390625e-08);
+                        }
+                    }
+                    team_bar(bar_id, nthreads);
+                    // ---- evaluation: group r takes residue r0 + r of the class ---------------------------------------------
+                    const int r = warp * gpw + grp;
+                    const bool active = r < S;
+                    const int c = o + (r0 + min(r, S - 1)) * sd, kk = 2 * c + par, split = c + par;
+                    const bool inert = (kk == 0) || (kk == n - 1);
+                    const int ilo = max(0, c - w_eff), jhi = min(L - 1, c + w_eff);
+                    const int nI = split - ilo, nJ = jhi - split + 1;
+                    float4 *cbn_r = cbn + (size_t)min(r, nspec - 1) * a.wpts, *cbo_r = cbo + (size_t)min(r, nspec - 1) * a.wpts;
+                    double p_dE = 0.0;
+                    if (active && !inert) {
+                        const Rot Rk = step_rot(kk, r);
+                        if (glane == 0) {
+#pragma unroll
+                            for (int q = 0; q < 9; ++q) rot_s[12 * r + q] = Rk.r[q];
+#pragma unroll
+                            for (int q = 0; q < 3; ++q) rot_s[12 * r + 9 + q] = Rk.t[q];
+                        }
+                        for (int jj = glane; jj < nJ; jj += gl) {
+                            const int j = split + jj;
+                            double x0, y0, z0, x, y, z;
+                            if (cb64) { x0 = X[3 * L + j]; y0 = Y[3 * L + j]; z0 = Z[3 * L + j]; }
+                            else cb_point(m, X, Y, Z, L, j, x0, y0, z0);
+                            rot_apply(Rk, x0, y0, z0, x, y, z);
+                            const float ct = __int_as_float(col_term<RING>(tb, j));
+                            cbn_r[jj] = make_float4((float)x, (float)y, (float)z, ct);
+                            const float4 cur = cb4[j];
+                            cbo_r[jj] = make_float4(cur.x, cur.y, cur.z, ct);
+                        }
+                    }
+                    __syncwarp();
+                    if (active && !inert)
+                        p_dE = (double)local_new_sum<RING>(m, tb, cb4, cbn_r, ilo, split, nI, nJ, glane, gl)
+                             - (double)local_new_sum<RING>(m, tb, cb4, cbo_r, ilo, split, nI, nJ, glane, gl);
+                    for (int d = gl >> 1; d > 0; d >>= 1) p_dE += __shfl_xor_sync(0xffffffffu, p_dE, d);
+                    if (active && glane == 0) sp_new[r] = p_dE;
+                    team_bar(bar_id, nthreads);
+                    // ---- decisions: lane q holds step q of the pass; all of them stand ---------------------------------------
+                    const int cq = o + (r0 + min(lane, S - 1)) * sd, kq = 2 * cq + par;
+                    const bool inert_q = (kq == 0) || (kq == n - 1);
+                    double dE = (lane < S && !inert_q) ? sp_new[lane] : 0.0;
+                    const double lu = b_lu[min(lane, S - 1)];
+                    const bool unc = lane < S && !inert_q && fabs(lu + dE * invT) < guard;
+                    bool acc = lane < S && (lu <= -dE * invT);
+                    unsigned m_unc = __ballot_sync(0xffffffffu, unc), m_exact = 0;
+                    while (m_unc) {
+                        const int r1 = __ffs(m_unc) - 1;
+                        const int cx = o + (r0 + r1) * sd, kx = 2 * cx + par;
+                        const double dx = team_sum(exact_dE_partial(exact_model(m), X, Y, Z, cb64 ? 1 : 0, kx, b_cd[r1], b_sd[r1],
+                                                                    max(0, cx - w_eff), min(L - 1, cx + w_eff), tid, nthreads),
+                                                   red, warp, nwarps, lane, bar_id);
+                        const bool ax = b_lu[r1] <= -dx / T;
+                        if (lane == r1) { dE = dx; acc = ax; }
+                        m_exact |= 1u << r1;
+                        m_unc &= ~(1u << r1);
+                    }
+                    const unsigned m_acc = __ballot_sync(0xffffffffu, acc);
+                    if (warp == 0 && lane < S) {
+                        const long long q = (t - a.sweep_offset) * n + pos_class + 2 * (r0 + lane) + par;
+                        if (q < a.trace_steps) {
+                            const size_t z = (size_t)row * a.trace_steps + q;
+                            if (a.trace_prop) a.trace_prop[z] = b_sp[lane];
+                            if (a.trace_dE) a.trace_dE[z] = dE;
+                            if (a.trace_acc) a.trace_acc[z] = (unsigned char)((acc ? 1 : 0) | (((m_exact >> lane) & 1u) ? 2 : 0));
+                        }
+                    }
+                    acc_l += (unsigned long long)__popc(m_acc);
+                    // ---- commit: the accepted rotations (all given in the frame before the pass) compose from the left:
+                    // a residue right of the accepted bonds c_1 < ... < c_j moves by M_j = R_1 R_2 ... R_j -----------------------
+                    if (tid == 0) {
+                        Xf cum = xf_identity();
+                        for (unsigned mm = m_acc; mm; mm &= mm - 1) {
+                            const int r1 = __ffs(mm) - 1;
+                            const int k1 = 2 * (o + (r0 + r1) * sd) + par;
+                            s[k1] = b_sp[r1];
+                            if (k1 == 0 || k1 == n - 1) { for (int q = 0; q < 9; ++q) rot_s[12 * r1 + q] = cum.r[q]; for (int q = 0; q < 3; ++q) rot_s[12 * r1 + 9 + q] = cum.t[q]; continue; }
+                            Xf Rr;
+                            for (int q = 0; q < 9; ++q) Rr.r[q] = rot_s[12 * r1 + q];
+                            for (int q = 0; q < 3; ++q) Rr.t[q] = rot_s[12 * r1 + 9 + q];
+                            cum = xf_mul(cum, Rr);
+                            for (int q = 0; q < 9; ++q) rot_s[12 * r1 + q] = cum.r[q];
+                            for (int q = 0; q < 3; ++q) rot_s[12 * r1 + 9 + q] = cum.t[q];
+                        }
+                    }
+                    team_bar(bar_id, nthreads);
+                    if (m_acc) {
+                        const int first = __ffs(m_acc) - 1;
+                        const int res0 = o + (r0 + first) * sd;                       // the leftmost residue that may move
+                        for (int res = res0 + tid; res < L; res += nthreads) {
+                            // the accepted move that governs this residue: the last one with c_r <= res (phi) or c_r < res (psi)
+                            int jr = -1, jprev = -1;
+                            for (unsigned mm = m_acc; mm; mm &= mm - 1) {
+                                const int r1 = __ffs(mm) - 1;
+                                const int c1 = o + (r0 + r1) * sd;
+                                if (c1 + par <= res) { jprev = jr; jr = r1; }
+                            }
+                            if (jr < 0) continue;
+                            const int cj = o + (r0 + jr) * sd;
+                            const bool on_axis = (par == 0 && res == cj) && !(2 * cj == 0);      // phi_c: N_c and CA_c stay with the left side
+#pragma unroll
+                            for (int at = 0; at < 4; ++at) {
+                                if (at == 3 && !cb64) break;
+                                const int jm = (on_axis && at < 2) ? jprev : jr;
+                                if (jm < 0) continue;
+                                Rot Mj;
+#pragma unroll
+                                for (int q = 0; q < 9; ++q) Mj.r[q] = rot_s[12 * jm + q];
+#pragma unroll
+                                for (int q = 0; q < 3; ++q) Mj.t[q] = rot_s[12 * jm + 9 + q];
+                                const int f = at * L + res;
+                                double x, y, z;
+                                rot_apply(Mj, X[f], Y[f], Z[f], x, y, z);
+                                X[f] = x; Y[f] = y; Z[f] = z;
+                            }
+                            double x, y, z;
+                            if (cb64) { x = X[3 * L + res]; y = Y[3 * L + res]; z = Z[3 * L + res]; }
+                            else cb_point(m, X, Y, Z, L, res, x, y, z);
+                            cb4[res] = make_float4((float)x, (float)y, (float)z, row_term(res));
+                        }
+                    }
+                    team_bar(bar_id, nthreads);
+                  }
+                }
+                pos_class += 2 * cnt;
+            }
+            k = n;                                                   // the sweep is done: skip Alg. 1's loop below
+        }
         while (k < n) {
             // ---- a1/a2: draws of the next 64 steps, two per lane (R5-R7) ----------------------------------
             if (k >= batch_end) {

@@ -551,6 +551,37 @@ def test_guard_off_is_fp32(amh, orc, torch, synth):
     assert np.all(np.abs(f["g"][diff]) < guard_bound(c.L, c.window, True))
 
 
+@pytest.mark.parametrize("wpc,cpc,gl,spec,stride", [(0, 0, 0, 0, 17), (2, 3, 8, 0, 17), (1, 1, 32, 0, 17), (4, 1, 16, 3, 17), (2, 7, 4, 0, 17),
+                                                    (0, 0, 0, 0, 5), (0, 0, 0, 0, 40), (3, 2, 8, 0, 1)])
+def test_strided_sweep_order_parity(amh, orc, torch, synth, wpc, cpc, gl, spec, stride):
+    # NEXT-4 (R26): local sweeps in the strided order.  stride >= 2w + 1 = 17: a class's proposals are evaluated in parallel
+    # (nothing speculative); smaller strides run the same order one proposal at a time; stride 1 is Alg. 1's order.  The
+    # oracle walks the order sequentially: every decision must be its own, the states identical, for every launch shape.
+    c = gi.CONFIGS[0]
+    ref, p, edges, m = synth(c.L, c.cfg_seed)
+    g = amh.AMH(p, edges, amh.default_options(warps_per_chain=wpc, chains_per_cta=cpc, lanes_per_step=gl, spec_local=spec))
+    s0 = gi.initial_states(c.B, c.n, seed=2)
+    st = torch.from_numpy(s0.copy()).cuda()
+    sweeps = 5
+    steps = sweeps * c.n
+    kw = dict(n_global=1, n_local=3, window=c.window, seed=4, local_stride=stride)
+    r = g.run(st, sweeps, trace_steps=steps, **kw)
+    chk = _follow_check(m, s0, r, steps, **kw)
+    assert chk["n_diff"] == 0
+    assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+    free = m.run(s0, sweeps, **kw)
+    assert np.array_equal(free["states"], st.cpu().numpy())
+    assert np.array_equal(free["n_accept_local"], r["n_accept_local"].cpu().numpy())
+    assert np.array_equal(free["n_accept_global"], r["n_accept_global"].cpu().numpy())
+    e = r["energy"].cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(e - free["energy"]) < 1e-5 * np.abs(free["energy"]))
+    if stride == 1:
+        plain = g.run(torch.from_numpy(s0.copy()).cuda(), sweeps, **dict(kw, local_stride=0))
+        assert np.array_equal(plain["energy"].cpu().numpy(), r["energy"].cpu().numpy())
+    print("strided order, stride %d, shape (%d, %d, %d, %d): %d steps, max |dE - oracle| %.2e, fp64-path steps %d"
+          % (stride, wpc, cpc, gl, spec, chk["err"].size, chk["err"][~chk["exact"]].max(), chk["exact"].sum()))
+
+
 def test_config0_in_full_follow_mode(amh, orc, torch, synth, gpu_model):
     # config 0 IN FULL (32 chains x 2,200 sweeps x 128 = 281,600 proposals per chain) replayed by the oracle in follow
     # mode: proposals bit-identical, every decision the oracle's except where its own gap is |g| < 1e-4 (logged), the

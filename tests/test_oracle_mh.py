@@ -335,3 +335,60 @@ def test_replica_exchange_keeps_each_temperature_boltzmann_L4(orc, synth):
     Te = np.ones(8, np.float32)
     Tn, acc, gap = orc.exchange(np.arange(8, dtype=np.float32), Te, 4, 1, 3)
     assert list(acc.keys()) == [1, 5] and list(acc.values()) == [1, 1] and np.array_equal(Tn, Te)   # odd cycle: pair (1, 2) of each group
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4: the strided sweep order (a variant of Alg. 1; R26)
+# ---------------------------------------------------------------------------------------------
+def test_strided_order_is_a_permutation_in_colour_classes(orc):
+    for L, s in ((10, 4), (64, 17), (7, 25), (33, 1)):
+        order = orc.sweep_order(L, False, s)
+        assert sorted(order.tolist()) == list(range(2 * L))                       # every variable once per sweep
+        res = order[0::2] // 2
+        assert np.array_equal(order[1::2], order[0::2] + 1) and np.all(order[0::2] % 2 == 0)     # phi_c, then psi_c
+        cls = res % s
+        assert np.all(np.diff(cls) >= 0)                                           # classes o = 0, 1, ... in turn
+        for o in range(min(s, L)):
+            assert np.array_equal(res[cls == o], np.arange(o, L, s))               # c = o, o + s, o + 2s, ...
+        assert np.array_equal(orc.sweep_order(L, True, s), np.arange(2 * L))       # global sweeps keep Alg. 1's order
+    assert np.array_equal(orc.sweep_order(12, False, 0), np.arange(24))
+    assert np.array_equal(orc.sweep_order(12, False, 1), np.arange(24))            # stride 1 IS Alg. 1's order
+
+
+def test_strided_run_with_stride_1_is_alg1_and_proposals_of_a_class_do_not_interact(orc, synth):
+    L, w = 40, 3
+    ref, p, edges, m = synth(L, 1000)
+    s0 = gi.initial_states(6, 2 * L, seed=3)
+    kw = dict(n_global=0, n_local=1, window=w, seed=11)
+    a = m.run(s0, 3, **kw); b = m.run(s0, 3, local_stride=1, **kw)
+    assert np.array_equal(a["states"], b["states"])
+    # one strided local sweep, traced; stride 2w + 1: the windows of a class are disjoint
+    sd = 2 * w + 1
+    n = 2 * L
+    r = m.run(s0, 1, local_stride=sd, trace_steps=n, **kw)
+    order = orc.sweep_order(L, False, sd)
+    assert not np.array_equal(r["states"], a["states"])                            # a different trajectory than Alg. 1's
+    # R26: inside a class every decision can be taken against the state at the START of the class (phi) or after the
+    # class's phi moves (psi): an accepted move turns everything right of it rigidly and leaves other windows' internal
+    # distances alone.  Checked with the oracle's own V_local (pin P5) on reconstructed states.
+    for row in range(2):
+        s = s0[row].copy()
+        pos = 0
+        for o in range(sd):
+            cs = list(range(o, L, sd))
+            for par in (0, 1):
+                base = s.copy()                                                     # state at the start of this half-class
+                for idx, c in enumerate(cs):
+                    q = pos + 2 * idx + par
+                    k = 2 * c + par
+                    assert order[q] == k
+                    t = base.copy(); t[k] = r["trace_prop"][row, q]
+                    want = m.energy_local(t, k, w) - m.energy_local(base, k, w)
+                    assert abs(r["trace_dE"][row, q] - want) < 1e-8, (o, par, c)
+                    if r["trace_acc"][row, q]:
+                        s[k] = r["trace_prop"][row, q]
+            pos += 2 * len(cs)
+        assert np.array_equal(s, r["states"][row])
+    # follow mode walks the same order
+    f = m.follow(s0, n, r["trace_acc"], local_stride=sd, **kw)
+    assert np.array_equal(f["states"], r["states"]) and np.array_equal(f["prop"], r["trace_prop"]) and np.array_equal(f["dE"], r["trace_dE"])
