@@ -182,8 +182,9 @@ def measured_peaks():
 
 
 def profiled_per_proposal(cfg_name: str, key: str):
-    """bytes per proposal of the sweep kernel from the committed ncu --set full summaries (profiles/r2_traffic.txt:
-    `<cfg> <key> = <value>`), or None.  key = dram_bytes_per_proposal | l2_bytes_per_proposal."""
+    """a figure of the sweep kernel from the committed ncu --set full summaries (profiles/r2_traffic.txt:
+    `<cfg> <key> = <value>`), or None.  key = dram_bytes_fixed | dram_bytes_per_proposal | l2_bytes_per_proposal |
+    thread_inst_per_proposal."""
     path = os.path.join(ROOT, "profiles", "r2_traffic.txt")
     try:
         for line in open(path):
@@ -334,11 +335,14 @@ class Workload:
         lanes = FP64_LANES_PER_SM if fp64 else FP32_LANES_PER_SM
         peak = n_sm * lanes * sm_max_mhz * 1e6 / 1e9          # Glane-op/s
         achieved = pair_evals * ops / (ms_per_step * 1e-3) / 1e9
-        dram = profiled_per_proposal(cfg.name, "dram_bytes_per_proposal")
+        dram_f = profiled_per_proposal(cfg.name, "dram_bytes_fixed")
+        dram_p = profiled_per_proposal(cfg.name, "dram_bytes_per_proposal")
+        dram = None if dram_f is None else dram_f + (dram_p or 0.0) * cfg.proposals
         l2b = profiled_per_proposal(cfg.name, "l2_bytes_per_proposal")
         r = dict(bound="alu", achieved=achieved, peak=peak, unit="Glane-op/s", frac=achieved / peak,
-                 traffic=(dram * cfg.proposals) if dram is not None else None,
-                 traffic_source="dram bytes per proposal of the ncu --set full capture of this config's kernel (profiles/r2_traffic.txt) x proposals per launch",
+                 traffic=dram,
+                 traffic_source="dram__bytes_read + dram__bytes_write of the ncu --set full capture of this config's kernel (profiles/r2_traffic.txt): "
+                                "a fixed first touch of the tables where they stay in L2, bytes per proposal x proposals where they do not (configs 3, 4)",
                  kernel=self.kernel_label(), pair_evals_per_launch=pair_evals, lane_ops_per_pair_eval=ops,
                  lane_ops_by_pipe=None if fp64 else LANE_OPS_BY_PIPE, pair_evals_per_s=pair_evals / (ms_per_step * 1e-3),
                  peak_source="derived: %d SMs x %d %s lanes x %.0f MHz (clocks.max.sm)" % (n_sm, lanes, "fp64" if fp64 else "fp32", sm_max_mhz),

@@ -294,6 +294,12 @@ amh_status amh_probe_gather(long long bytes, int reps, double *gathers_per_s, vo
  * shared memory, nspec = local proposals per pass, lanes = lanes per local proposal.  Any pointer may be NULL.  Host. */
 amh_status amh_launch_variant(amh_ctx *ctx, long long B, int window, int *spec_global, int *ring, int *cb64, int *nspec, int *lanes);
 
+/* Checked build only (python -m paper_2211_03193_b200.build --checked: every table, ring and shared-memory index of the
+ * pair loops is range-checked on the device): *code = 0 if no check has failed since the library was loaded, else the
+ * largest code of a failed check; *checked = 1 in a checked build, 0 in the product build (whose *code stays 0).
+ * Synchronises the device.  Host outputs. */
+amh_status amh_check_status(int *code, int *checked);
+
 const char *amh_last_error(void);
 const char *amh_version(void);
 

@@ -25,7 +25,7 @@ PROP_UNIFORM, PROP_GRID, PROP_GAUSSIAN = 0, 1, 2
 # every symbol include/amh.h declares
 EXPORTS = ["amh_default_options", "amh_default_launch_options", "amh_set_launch_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
            "amh_create_tr5", "amh_pair_geometry", "amh_run", "amh_run_host", "amh_run_pt", "amh_exchange", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
-           "amh_probe_l2_read", "amh_probe_gather", "amh_launch_variant", "amh_last_error", "amh_version"]
+           "amh_probe_l2_read", "amh_probe_gather", "amh_launch_variant", "amh_check_status", "amh_last_error", "amh_version"]
 
 
 class AMHError(RuntimeError):
@@ -132,6 +132,7 @@ def lib():
         L.amh_probe_l2_read.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_double), C.c_void_p]
         L.amh_probe_gather.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_double), C.c_void_p]
         L.amh_launch_variant.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 5
+        L.amh_check_status.argtypes = [C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.amh_philox_test.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]
         L.amh_default_options.argtypes = [C.POINTER(_ModelOptions)]
         L.amh_default_launch_options.argtypes = [C.POINTER(_LaunchOptions)]
@@ -174,6 +175,13 @@ def _dev(t, dtype, name):
     if t.dtype != dtype or not t.is_cuda or not t.is_contiguous():
         t = t.to(device="cuda", dtype=dtype).contiguous()
     return t
+
+
+def check_status():
+    """amh_check_status: (code of the largest failed device-side range check or 0, whether this is the checked build)."""
+    a, b = C.c_int(), C.c_int()
+    _check(lib().amh_check_status(C.byref(a), C.byref(b)))
+    return a.value, bool(b.value)
 
 
 def probe_l2_read(n_bytes: int, reps: int = 20) -> float:

@@ -47,6 +47,23 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps())
 
 
+LIB_CHECKED = os.path.join(CSRC, "libamh_b200_checked.so")
+
+
+def build_checked(force: bool = False) -> str:
+    """The same library with -DAMH_CHECK: device-side range checks on every table / ring / shared-memory index of the
+    pair loops (amh_check_status reports a failure).  For tests; the product path loads LIB."""
+    if force or not os.path.exists(LIB_CHECKED) or any(os.path.getmtime(d) > os.path.getmtime(LIB_CHECKED) for d in deps()):
+        tmp = LIB_CHECKED + ".tmp%d" % os.getpid()
+        cmd = [nvcc()] + [f for f in NVCC_FLAGS if f not in ("-Xptxas", "-v")] + ["-DAMH_CHECK", "-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            sys.stderr.write(r.stdout + r.stderr)
+            raise RuntimeError("nvcc failed: " + " ".join(cmd))
+        os.replace(tmp, LIB_CHECKED)
+    return LIB_CHECKED
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         tmp = LIB + ".tmp%d" % os.getpid()
@@ -64,4 +81,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
+    if "--checked" in sys.argv:
+        print(build_checked(force="--force" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose=True))

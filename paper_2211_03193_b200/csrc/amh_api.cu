@@ -956,6 +956,21 @@ amh_status amh_probe_gather(long long bytes, int reps, double *gathers_per_s, vo
     return AMH_OK;
 }
 
+amh_status amh_check_status(int *code, int *checked)
+{
+    if (!code || !checked) return fail(AMH_ERR_INVALID_ARG, "amh_check_status: output is NULL");
+#ifdef AMH_CHECK
+    *checked = 1;
+#else
+    *checked = 0;
+#endif
+    int v = 0;
+    AMH_CUDA(cudaDeviceSynchronize());
+    AMH_CUDA(cudaMemcpyFromSymbol(&v, amh::amh_check_word, sizeof(int)));
+    *code = v;
+    return AMH_OK;
+}
+
 amh_status amh_philox_test(const unsigned int *ctr, const unsigned int *key, unsigned int *out, long long count, void *cuda_stream)
 {
     if (count < 0 || (count > 0 && (!ctr || !key || !out))) return fail(AMH_ERR_INVALID_ARG, "amh_philox_test: bad arguments");

@@ -39,6 +39,16 @@
 #include "amh_device.cuh"
 
 namespace amh {
+// Checked build (-DAMH_CHECK, `python -m paper_2211_03193_b200.build --checked`): every table / ring / shared-memory index the
+// pair loops form is range-checked and a violation leaves its code in a device word that amh_check_status() returns.
+// (compute-sanitizer is closed on the GPU pool this was developed on; tests/test_gpu_checked.py runs the launch shapes of
+// the parity tests through this build instead.)  The product build compiles the checks out.
+__device__ int amh_check_word = 0;
+#ifdef AMH_CHECK
+#define AMH_ASSERT(cond, code) do { if (!(cond)) atomicMax(&amh_check_word, (code)); } while (0)
+#else
+#define AMH_ASSERT(cond, code) ((void)0)
+#endif
 #ifndef AMH_UL
 #define AMH_UL 3
 #endif
@@ -237,6 +247,7 @@ struct LocalTab {
     int ring_cols, ring_rows, min_sep, stride4;              // stride4 = row_stride * 4 (RING)
     int slot_c, c_ref;                                       // ring slot of column c_ref (RING)
     int nb8;                                                 // nb * 8 (L2)
+    long long lo, hi;                                        // checked build: valid byte offsets from base are [lo, hi)
 };
 
 template <bool RING>
@@ -260,6 +271,9 @@ __device__ __forceinline__ float local_pair(const DevModel &m, const LocalTab &t
     float f;
     bin_frac(d2, m.t0, m.inv_delta, m.tmax, m.thmax, b, f);
     const unsigned char *row = tb.base + (__float_as_int(ci.w) + __float_as_int(pj.w));
+    AMH_ASSERT(b >= 0 && b <= m.nb - 2, 1);
+    AMH_ASSERT((long long)(__float_as_int(ci.w) + __float_as_int(pj.w)) + (long long)b * (RING ? 4 : 8) >= tb.lo &&
+               (long long)(__float_as_int(ci.w) + __float_as_int(pj.w)) + (long long)(b + 1) * (RING ? 4 : 8) + (RING ? 4 : 0) <= tb.hi, 2);
     if (RING) {
         const float *r = reinterpret_cast<const float *>(row) + b;
         const float e0 = r[0], e1 = r[1];
@@ -289,6 +303,7 @@ __device__ __forceinline__ float local_new_sum(const DevModel &m, const LocalTab
         for (int u = 0; u < U; ++u) {
             const bool in = p + u * gl < nP;
             const int iu = in ? ii : 0, ju = in ? jj : 0;
+            AMH_ASSERT(ilo + iu >= 0 && ilo + iu < m.L && ju >= 0 && ju < nJ, 3);
             const float4 ci = cb4[ilo + iu];
             const float4 pj = cbn[ju];
             const bool valid = in && (split + ju) - (ilo + iu) >= m.min_sep;
@@ -349,6 +364,7 @@ __device__ __forceinline__ float local_transition(const DevModel &m, const Local
         const int t = isl ? q : q - lv.cnt;
         const int i = isl ? lv.i0 + t * lv.di : en.i0 + t * en.di;
         const int j = isl ? lv.j0 + t * lv.dj : en.j0 + t * en.dj;
+        AMH_ASSERT(i >= 0 && i < j && j < m.L && j - i >= m.min_sep, 4);
         const float4 ci = cb4[i];
         float4 cj = cb4[j];
         cj.w = __int_as_float(col_term<RING>(tb, j));
@@ -423,6 +439,7 @@ __device__ __forceinline__ double global_cols_sum(const DevModel &m, const float
                         if (near[u]) {
                             int bn;
                             bin_frac(d2[u], m.t0, m.inv_delta, m.tmax, m.thmax, bn, f[u]);
+                            AMH_ASSERT(bn >= 0 && bn <= m.nb - 2 && i + u >= 0 && i + u < j && j < m.L, 5);
                             v[u] = __ldg(m.Epk + (size_t)tri_row(i + u, j, m.L) * m.nb + bn);
                         }
                     }
@@ -688,6 +705,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the teams' reads of the old column come first
                 if (nrows > 0) {
                     mbar_expect_tx(bar, (uint32_t)nrows * row_bytes);
+                    AMH_ASSERT(nrows <= a.ring_rows && nrows <= m.band_rows && s >= 0 && s < R, 6);
                     tma_bulk_g2s(ring + (size_t)s * a.ring_rows * m.row_stride, m.Ebd + (size_t)j * m.band_rows * m.row_stride,
                                  (uint32_t)nrows * row_bytes, bar);
                 } else {
@@ -749,6 +767,8 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     tb.base = use_ring ? reinterpret_cast<const unsigned char *>(ring) : reinterpret_cast<const unsigned char *>(m.Epk);
     tb.ring_cols = R; tb.ring_rows = a.ring_rows; tb.min_sep = m.min_sep; tb.stride4 = m.row_stride * 4; tb.nb8 = m.nb * 8;
     tb.slot_c = 0; tb.c_ref = 0;
+    tb.lo = use_ring ? -(long long)kRingPadRows * m.row_stride * 4 : 0;
+    tb.hi = use_ring ? (long long)R * a.ring_rows * m.row_stride * 4 : (long long)((size_t)L * (L - 1) / 2) * m.nb * 8;
 
     // the bond the torsion k turns about: phi_c N->CA, psi_c CA->C
     auto step_rot = [&](int k, int bi) -> Rot {
@@ -1116,6 +1136,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                             if (cb64) { x0 = X[3 * L + j]; y0 = Y[3 * L + j]; z0 = Z[3 * L + j]; }
                             else cb_point(m, X, Y, Z, L, j, x0, y0, z0);
                             rot_apply(Rk, x0, y0, z0, x, y, z);
+                            AMH_ASSERT(jj < a.wpts && r < nspec && j < L, 7);
                             cbn_r[jj] = make_float4((float)x, (float)y, (float)z, __int_as_float(col_term<RING>(tb, j)));
                         }
                     }
