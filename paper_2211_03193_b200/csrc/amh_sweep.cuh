@@ -91,6 +91,7 @@ constexpr int kDrawBatch = 64;           // steps whose draws are generated toge
 constexpr int kMaxWarps = 16;            // array bound of the per-warp scratch of a team
 constexpr int kMaxSpec = 16;             // proposals evaluated per pass, at most
 constexpr int kBlk = 8;                  // residues per culling block of the global phase
+constexpr int kSup = 4;                  // blocks per super-block (second culling level)
 constexpr int kMaxTeamWarps = 15;        // team warps per CTA: chains x warps per chain (+ the producer = 512 threads)
 constexpr int kMaxChains = 15;           // chains per CTA (named barriers 1..15)
 constexpr int kSweepMaxThreads = 512;    // 15 team warps + the producer: 128 registers per thread
@@ -103,7 +104,8 @@ constexpr int kRingPadRows = 4;          // rows in front of the first ring slot
 //   double red[32], b_cd[64], b_sd[64], b_lu[64], rot_s[16][12], sp_new[16], sp_T[16]
 //   float4 cb4[L]                fp32 copy of the C-betas (what the pair loops read); .w = byte offset of the
 //                                residue's term in a table address (as the ROW index i of a pair)
-//   float4 blk4[ceil(L/8)]       bounding spheres of 8-residue blocks (culling in the global phase)
+//   float4 blk4[ceil(L/8) + ceil(L/32)]   bounding spheres of the 8-residue blocks, then of the 32-residue super-blocks
+//                                (two-level culling in the global phase)
 //   float4 cbn[nspec][wpts]      the turned C-betas of the local proposals of a pass; .w = the column's term
 //   float  s[n], b_sp[64]
 __host__ __device__ inline size_t chain_smem_bytes(int L, int cb64, int nspec, int wpts, int W)
@@ -111,7 +113,8 @@ __host__ __device__ inline size_t chain_smem_bytes(int L, int cb64, int nspec, i
     size_t doubles = (cb64 ? 12 : 9) * (size_t)L;
     doubles += doubles & 1;                                  // float4 arrays on 16 bytes
     doubles += 2 * kMaxWarps + 3 * kDrawBatch + 12 * kMaxSpec + 2 * kMaxSpec;
-    size_t floats = 4 * (size_t)L + 4 * (((size_t)L + kBlk - 1) / kBlk) + 4 * (size_t)nspec * wpts + 2 * (size_t)L + kDrawBatch;
+    const size_t nblk = ((size_t)L + kBlk - 1) / kBlk;
+    size_t floats = 4 * (size_t)L + 4 * (nblk + (nblk + kSup - 1) / kSup) + 4 * (size_t)nspec * wpts + 2 * (size_t)L + kDrawBatch;
     floats = (floats + 3) & ~(size_t)3;
     return sizeof(double) * doubles + sizeof(float) * floats;
 }
@@ -409,7 +412,22 @@ __device__ __forceinline__ double global_cols_sum(const DevModel &m, const float
         }
         const int i_end = min(split - 1, j - m.min_sep);
         const int nblk = i_end < 0 ? 0 : i_end / kBlk + 1;
-        for (int b = slice; b < nblk; b += S) {
+        const int nblk_all = (m.L + kBlk - 1) / kBlk;
+        int b = slice;
+        while (b < nblk) {
+            // second culling level: a super-block of kSup blocks beyond the last bin centre is skipped whole
+            const int sb = b / kSup;
+            if (nblk_all > 4 * kSup) {                                      // long chains only: short ones have too few blocks to gain
+                const float4 sl = blk4[nblk_all + sb];
+                const float dx = sl.x - xn, dy = sl.y - yn, dz = sl.z - zn;
+                if (fmaf(dx, dx, fmaf(dy, dy, dz * dz)) >= sl.w) {
+                    const int nb0 = (sb + 1) * kSup;                       // this slice's first block at or after nb0
+                    b = (S == 1) ? nb0 : slice + small_div(max(nb0 - slice, 0) + S - 1, S) * S;
+                    continue;
+                }
+            }
+            const int bend = min(nblk, (sb + 1) * kSup);
+            for (; b < bend; b += S) {
             const float4 bl = blk4[b];
             {
                 const float dx = bl.x - xn, dy = bl.y - yn, dz = bl.z - zn;
@@ -448,6 +466,7 @@ __device__ __forceinline__ double global_cols_sum(const DevModel &m, const float
                 }
             }
             acc += (double)part;
+            }
         }
     }
     return acc;
@@ -594,8 +613,7 @@ __device__ __forceinline__ float team_extent(const float4 *cb4, int L, double *r
 __device__ __forceinline__ void team_blocks(const DevModel &m, const float4 *cb4, float4 *blk4, int first, int tid, int nthr)
 {
     const int nblk = (m.L + kBlk - 1) / kBlk;
-    for (int b = first + tid; b < nblk; b += nthr) {
-        const int lo = b * kBlk, hi = min(m.L, lo + kBlk);
+    auto sphere = [&](int lo, int hi) -> float4 {
         float cx = 0.0f, cy = 0.0f, cz = 0.0f;
         for (int i = lo; i < hi; ++i) { const float4 c = cb4[i]; cx += c.x; cy += c.y; cz += c.z; }
         const float inv = 1.0f / (float)(hi - lo);
@@ -607,8 +625,13 @@ __device__ __forceinline__ void team_blocks(const DevModel &m, const float4 *cb4
             r2 = fmaxf(r2, fmaf(dx, dx, fmaf(dy, dy, dz * dz)));
         }
         const float t = (m.dfar + sqrtf(r2)) * 1.00001f + 1e-4f;
-        blk4[b] = make_float4(cx, cy, cz, t * t);
-    }
+        return make_float4(cx, cy, cz, t * t);
+    };
+    for (int b = first + tid; b < nblk; b += nthr) blk4[b] = sphere(b * kBlk, min(m.L, (b + 1) * kBlk));
+    // the super-blocks of kSup blocks each, from the points themselves (the last threads take them, so that both levels run at once)
+    const int nsup = (nblk + kSup - 1) / kSup;
+    for (int sb = first / kSup + (nthr - 1 - tid); sb < nsup; sb += nthr)
+        blk4[nblk + sb] = sphere(sb * kSup * kBlk, min(m.L, (sb + 1) * kSup * kBlk));
 }
 
 // V (Eq. 3a) of the team's chain from its fp32 C-betas: v_far (every pair at its clamped value) + the excess of the
@@ -728,7 +751,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     double *rot_s = b_lu + kDrawBatch, *sp_new = rot_s + 12 * kMaxSpec, *sp_T = sp_new + kMaxSpec;
     float4 *cb4 = reinterpret_cast<float4 *>(sp_T + kMaxSpec);
     float4 *blk4 = cb4 + L;
-    float4 *cbn = blk4 + (L + kBlk - 1) / kBlk;
+    float4 *cbn = blk4 + (L + kBlk - 1) / kBlk + ((L + kBlk - 1) / kBlk + kSup - 1) / kSup;
     float *s = reinterpret_cast<float *>(cbn + (size_t)cbn_rows * a.wpts);
     float *b_sp = s + n;
 
