@@ -107,14 +107,14 @@ constexpr int kRingPadRows = 4;          // rows in front of the first ring slot
 //   float4 blk4[ceil(L/8) + ceil(L/32)]   bounding spheres of the 8-residue blocks, then of the 32-residue super-blocks
 //                                (two-level culling in the global phase)
 //   float4 cbn[nspec][wpts]      the turned C-betas of the local proposals of a pass; .w = the column's term
-//   float  s[n], b_sp[64]
+//   float  s[n], b_sp[64];  int ctr[4]  (chunk counter of the whole-team global proposals)
 __host__ __device__ inline size_t chain_smem_bytes(int L, int cb64, int nspec, int wpts, int W)
 {
     size_t doubles = (cb64 ? 12 : 9) * (size_t)L;
     doubles += doubles & 1;                                  // float4 arrays on 16 bytes
     doubles += 2 * kMaxWarps + 3 * kDrawBatch + 12 * kMaxSpec + 2 * kMaxSpec;
     const size_t nblk = ((size_t)L + kBlk - 1) / kBlk;
-    size_t floats = 4 * (size_t)L + 4 * (nblk + (nblk + kSup - 1) / kSup) + 4 * (size_t)nspec * wpts + 2 * (size_t)L + kDrawBatch;
+    size_t floats = 4 * (size_t)L + 4 * (nblk + (nblk + kSup - 1) / kSup) + 4 * (size_t)nspec * wpts + 2 * (size_t)L + kDrawBatch + 4;
     floats = (floats + 3) & ~(size_t)3;
     return sizeof(double) * doubles + sizeof(float) * floats;
 }
@@ -386,17 +386,28 @@ __device__ __forceinline__ float local_transition(const DevModel &m, const Local
 // every S-th block.
 __device__ __forceinline__ double global_cols_sum(const DevModel &m, const float4 *cb4, const float4 *blk4,
                                                   const double *X, const double *Y, const double *Z, bool cb64, bool turn, const Rot &R,
-                                                  int split, int jlo, int jhi, int tid, int nthr)
+                                                  int split, int jlo, int jhi, int tid_, int nthr_, int *ctr = nullptr)
 {
     const int nJ = jhi - jlo + 1;
     double acc = 0.0;
     if (split <= 0 || nJ <= 0) return acc;
-    for (int c0 = 0; c0 < nJ; c0 += nthr) {
+    // ctr (a shared-memory counter, 0 at entry; whole-team calls only): when there are at least as many columns as threads, the
+    // team's warps do not take fixed rounds of columns but GRAB chunks of 32 columns as they finish (culling makes the chunks
+    // uneven; with fixed rounds the fast warps wait at the reduction).  The sum does not depend on who takes which chunk.
+    const bool dyn = ctr != nullptr && nthr_ > 32 && nJ >= nthr_;
+    const int nthr = dyn ? 32 : nthr_, tid = dyn ? (tid_ & 31) : tid_;
+    for (int c0 = 0;; c0 += dyn ? 0 : nthr) {
+        if (dyn) {
+            int ch = 0;
+            if (tid == 0) ch = atomicAdd(ctr, 1);
+            c0 = __shfl_sync(0xffffffffu, ch, 0) * 32;
+        }
+        if (c0 >= nJ) break;
         const int nc = min(nthr, nJ - c0);
         int S = 1, col = tid, slice = 0;
         if (nc < nthr) {
             S = small_div(nthr, nc); slice = small_div(tid, nc); col = tid - slice * nc;
-            if (slice >= S) break;
+            if (slice >= S) { if (dyn) continue; else break; }
         }
         const int j = jlo + c0 + col;
         float xn, yn, zn;
@@ -754,11 +765,13 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
     float4 *cbn = blk4 + (L + kBlk - 1) / kBlk + ((L + kBlk - 1) / kBlk + kSup - 1) / kSup;
     float *s = reinterpret_cast<float *>(cbn + (size_t)cbn_rows * a.wpts);
     float *b_sp = s + n;
+    int *ctr = reinterpret_cast<int *>(b_sp + kDrawBatch);
 
     const long long row = row0 + slot;
     const unsigned long long chain = (unsigned long long)(a.chain_offset + row);
 
     for (int q = tid; q < n; q += nthreads) s[q] = a.states[row * n + q];
+    if (tid == 0) ctr[0] = 0;
     team_bar(bar_id, nthreads);
     // the row term of residue i in a local table address (see LocalTab)
     auto row_term = [&](int i) -> float {
@@ -1088,7 +1101,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
 #pragma unroll
                         for (int q = 0; q < 3; ++q) rot_s[9 + q] = Rk.t[q];
                     }
-                    p_new = global_cols_sum(m, cb4, blk4, X, Y, Z, cb64, true, Rk, split, split, L - 1, tid, nthreads);
+                    p_new = global_cols_sum(m, cb4, blk4, X, Y, Z, cb64, true, Rk, split, split, L - 1, tid, nthreads, ctr);
                 }
                 if (k & 1) {                                  // the split moved: column c leaves, row c enters
                     const int c = k >> 1;
@@ -1096,6 +1109,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                         - global_col_sum(m, cb4, c, c - m.min_sep + 1, tid, nthreads);
                 }
                 team_sum2(p_new, p_T, red, warp, nwarps, lane, bar_id);
+                if (tid == 0) ctr[0] = 0;                     // every warp is past its last grab; the pass ends with a barrier
                 my_new = p_new; my_T = p_T;
             } else {
                 if (use_ring && !gp) {
