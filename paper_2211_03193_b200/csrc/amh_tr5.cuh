@@ -13,8 +13,8 @@
 // and no decision guard is needed; the orientation terms do not vanish with distance, so nothing is culled either.
 // One CTA per chain, one proposal at a time by the whole CTA (Alg. 1 literally): a proposal turns the atoms right of the
 // flipped bond into a scratch copy, the pairs that straddle the bond (all of them, or those inside the window) are dealt
-// to the threads, new minus old, block reduction, Metropolis test, commit.  This row is built for parity and a first
-// number, not yet for speed.
+// to the threads (new state only: the old state's sum is carried from step to step as in amh_sweep.cuh), block reduction,
+// Metropolis test, commit.  This row is built for parity and a first number, not yet for speed.
 #pragma once
 #include "amh_device.cuh"
 #include "amh_sweep.cuh"
@@ -192,6 +192,18 @@ __device__ __forceinline__ double tr5_block_sum(double v, double *red)
     return tot;
 }
 
+// two sums at once
+__device__ __forceinline__ void tr5_block_sum2(double &a, double &b, double *red)
+{
+    a = warp_sum(a); b = warp_sum(b);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    if (lane == 0) { red[warp] = a; red[16 + warp] = b; }
+    __syncthreads();
+    a = 0.0; b = 0.0;
+    for (int w = 0; w < nw; ++w) { a += red[w]; b += red[16 + w]; }
+    __syncthreads();
+}
+
 // V restricted to residues lo..hi of the atoms in shared memory (every thread returns the total)
 __device__ __forceinline__ double tr5_energy_range(const Tr5Model &m, const double *A, double *red, int lo, int hi)
 {
@@ -315,6 +327,12 @@ __global__ void __launch_bounds__(128, 3) tr5_sweep_kernel(Tr5Model m, RunArgs a
             if (!(a.sigma_start == a.sigma_end || a.ramp_sigma <= 1 || t <= 0))
                 sigma_t = (t >= a.ramp_sigma - 1) ? a.sigma_end
                                                   : a.sigma_start + (a.sigma_end - a.sigma_start) * ((double)t / (double)(a.ramp_sigma - 1));
+            // dE = S_new - S_old over the straddling pairs; only S_new is summed pair by pair: S_old is carried from step to step
+            // by the row and the column that enter and leave the straddling set (transition_lines of amh_sweep.cuh on the
+            // equivalent (phi, psi) index k2: phi_c <-> 2c, psi_c and omega_c <-> 2c + 1, the same set for both) and becomes
+            // the accepted proposal's S_new
+            double S_prev = 0.0;
+            int k2_prev = 0;
             for (int k = 0; k < n; ++k) {
                 const int c = k / 5, slot = k - 5 * c;
                 const int split = c + (slot > 0 ? 1 : 0);
@@ -350,7 +368,7 @@ __global__ void __launch_bounds__(128, 3) tr5_sweep_kernel(Tr5Model m, RunArgs a
                     sh_lu = log((double)((x0 >> 8) + 1u) * 5.9604644775390625e-08);
                 }
                 __syncthreads();
-                double dE = 0.0;
+                double dE = 0.0, s_new_sum = 0.0;
                 Rot R;
                 if (!inert) {
                     // ---- a3: the bond the slot turns about: phi_c N_c -> CA_c, psi_c CA_c -> C_c, omega_c C_c -> N_{c+1} -------
@@ -370,17 +388,34 @@ __global__ void __launch_bounds__(128, 3) tr5_sweep_kernel(Tr5Model m, RunArgs a
                         o[0] = x; o[L] = y; o[2 * L] = z;
                     }
                     __syncthreads();
-                    // ---- a4/a5: straddling pairs, new minus old ------------------------------------------------------
+                    // ---- a4/a5: straddling pairs of the new state; the lines that enter / leave the set at the old one ------------
                     const int nI = split - ilo, nJ = jhi - split + 1;
-                    double part = 0.0;
+                    double part = 0.0, part_T = 0.0;
                     for (int idx = tid; idx < nI * nJ; idx += nthr) {
                         const int i = ilo + idx / nJ, j = split + idx % nJ;
                         if (j - i < m.min_sep) continue;
-                        const V3 Ni = tr5_atom(A, L, 0, i), CAi = tr5_atom(A, L, 1, i), CBi = tr5_atom(A, L, 3, i);
-                        part += tr5_pair(m, i, j, Ni, CAi, CBi, tr5_atom(Rn, L, 0, j), tr5_atom(Rn, L, 1, j), tr5_atom(Rn, L, 2, j))
-                              - tr5_pair(m, i, j, Ni, CAi, CBi, tr5_atom(A, L, 0, j), tr5_atom(A, L, 1, j), tr5_atom(A, L, 3, j));
+                        part += tr5_pair(m, i, j, tr5_atom(A, L, 0, i), tr5_atom(A, L, 1, i), tr5_atom(A, L, 3, i),
+                                         tr5_atom(Rn, L, 0, j), tr5_atom(Rn, L, 1, j), tr5_atom(Rn, L, 2, j));
                     }
-                    dE = tr5_block_sum(part, red);
+                    const int k2 = 2 * c + (slot > 0 ? 1 : 0);
+                    if (k2 != k2_prev) {                          // k2 = k2_prev + 1: one row and one column change hands
+                        Line lv, en;
+                        transition_lines(k2, L, gp ? L : min(a.window, L - 1), m.min_sep, lv, en);
+                        for (int q = tid; q < lv.cnt + en.cnt; q += nthr) {
+                            const bool isl = q < lv.cnt;
+                            const int tq = isl ? q : q - lv.cnt;
+                            const int i = isl ? lv.i0 + tq * lv.di : en.i0 + tq * en.di;
+                            const int j = isl ? lv.j0 + tq * lv.dj : en.j0 + tq * en.dj;
+                            const double e = tr5_pair(m, i, j, tr5_atom(A, L, 0, i), tr5_atom(A, L, 1, i), tr5_atom(A, L, 3, i),
+                                                      tr5_atom(A, L, 0, j), tr5_atom(A, L, 1, j), tr5_atom(A, L, 3, j));
+                            part_T += isl ? -e : e;
+                        }
+                    }
+                    tr5_block_sum2(part, part_T, red);
+                    S_prev += part_T;                             // S_old of this step's set for the current state
+                    k2_prev = k2;
+                    dE = part - S_prev;
+                    s_new_sum = part;
                 }
                 // ---- a7: Metropolis test (Eq. 1a/2a, R14), in fp64 like everything else here ------------------
                 const bool accept = sh_lu <= -dE / T;
@@ -395,6 +430,7 @@ __global__ void __launch_bounds__(128, 3) tr5_sweep_kernel(Tr5Model m, RunArgs a
                 }
                 if (accept) {
                     if (gp) ++acc_g; else ++acc_l;
+                    if (!inert) S_prev = s_new_sum;               // the accepted proposal's S_new is its set's S_old from now on
                     if (tid == 0) s[k] = sh_sp;
                     if (!inert) {
                         // every atom bonded after the turned bond moves: phi_c: C_c, CB_c and the residues after c;
