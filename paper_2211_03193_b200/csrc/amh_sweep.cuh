@@ -300,21 +300,23 @@ __device__ __forceinline__ float local_new_sum(const DevModel &m, const LocalTab
 #pragma unroll
     for (int u = 0; u < U; ++u) acc[u] = 0.0f;
     if (nP <= 0) return 0.0f;
-    int ii = small_div(glane, nJ), jj = glane - ii * nJ;
+    // p / nJ by a 32-bit reciprocal (one IMAD.HI per pair instead of carrying (i, j) along): exact for p * nJ < 2^32
+    const unsigned rcp = 0xffffffffu / (unsigned)nJ + 1u;
+    const bool one_col = nJ == 1;                            // 2^32 / 1 does not fit
+    const int dsep = split - ilo - m.min_sep;                // valid iff ju - iu + dsep >= 0
     for (int p = glane; p < nP; p += U * gl) {
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const bool in = p + u * gl < nP;
-            const int iu = in ? ii : 0, ju = in ? jj : 0;
-            AMH_ASSERT(ilo + iu >= 0 && ilo + iu < m.L && ju >= 0 && ju < nJ, 3);
+            const int q = p + u * gl;
+            const bool in = q < nP;
+            const int qq = in ? q : 0;
+            const int iu = one_col ? qq : (int)__umulhi((unsigned)qq, rcp), ju = qq - iu * nJ;
+            AMH_ASSERT(ilo + iu >= 0 && ilo + iu < m.L && ju >= 0 && ju < nJ && iu < nI, 3);
             const float4 ci = cb4[ilo + iu];
             const float4 pj = cbn[ju];
-            const bool valid = in && (split + ju) - (ilo + iu) >= m.min_sep;
+            const bool valid = in && ju - iu + dsep >= 0;
             const float e = local_pair<RING>(m, tb, ci, pj);
             acc[u] += valid ? e : 0.0f;
-            jj += gl;
-            if (jj >= nJ) { jj -= nJ; ++ii; }
-            while (jj >= nJ) { jj -= nJ; ++ii; }             // gl > nJ only at the chain ends
         }
     }
     float s = acc[0];
