@@ -149,9 +149,8 @@ __device__ __forceinline__ void mbar_arrive(void *bar)
 {
     asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
+__device__ __forceinline__ void mbar_wait_u32(uint32_t a, uint32_t parity)
 {
-    const uint32_t a = smem_u32(bar);
     uint32_t ok;
     do {
         // the last operand lets the hardware park the thread for up to ~1 us instead of spinning on the barrier
@@ -159,6 +158,7 @@ __device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
                      : "=r"(ok) : "r"(a), "r"(parity), "r"(1000u) : "memory");
     } while (!ok);
 }
+__device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity) { mbar_wait_u32(smem_u32(bar), parity); }
 // global -> shared bulk copy (TMA, no tensor map); bytes is a multiple of 16, both addresses 16-byte aligned
 __device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, uint32_t bytes, void *bar)
 {
@@ -362,21 +362,31 @@ __device__ __forceinline__ float local_transition(const DevModel &m, const Local
 {
     Line lv, en;
     transition_lines(k, m.L, w, m.min_sep, lv, en);
-    float acc = 0.0f;
+    float acc0 = 0.0f, acc1 = 0.0f;
     const int tot = lv.cnt + en.cnt;
-    for (int q = glane; q < tot; q += gl) {
-        const bool isl = q < lv.cnt;
-        const int t = isl ? q : q - lv.cnt;
-        const int i = isl ? lv.i0 + t * lv.di : en.i0 + t * en.di;
-        const int j = isl ? lv.j0 + t * lv.dj : en.j0 + t * en.dj;
-        AMH_ASSERT(i >= 0 && i < j && j < m.L && j - i >= m.min_sep, 4);
-        const float4 ci = cb4[i];
-        float4 cj = cb4[j];
-        cj.w = __int_as_float(col_term<RING>(tb, j));
-        const float e = local_pair<RING>(m, tb, ci, cj);
-        acc += isl ? -e : e;
+    // two pairs per lane and trip (the two lines hold 2 (w + 1) pairs at most, i.e. two trips of a group of 8)
+    for (int q0 = glane; q0 < tot; q0 += 2 * gl) {
+        float e[2];
+        bool isl[2], in[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int q = q0 + u * gl;
+            in[u] = q < tot;
+            const int qq = in[u] ? q : q0;
+            isl[u] = qq < lv.cnt;
+            const int t = isl[u] ? qq : qq - lv.cnt;
+            const int i = isl[u] ? lv.i0 + t * lv.di : en.i0 + t * en.di;
+            const int j = isl[u] ? lv.j0 + t * lv.dj : en.j0 + t * en.dj;
+            AMH_ASSERT(i >= 0 && i < j && j < m.L && j - i >= m.min_sep, 4);
+            const float4 ci = cb4[i];
+            float4 cj = cb4[j];
+            cj.w = __int_as_float(col_term<RING>(tb, j));
+            e[u] = local_pair<RING>(m, tb, ci, cj);
+        }
+        acc0 += isl[0] ? -e[0] : e[0];
+        acc1 += in[1] ? (isl[1] ? -e[1] : e[1]) : 0.0f;
     }
-    return acc;
+    return acc0 + acc1;
 }
 
 // ---- global phase -------------------------------------------------------------------------------------------
@@ -653,29 +663,36 @@ __device__ __forceinline__ double team_full_energy(const DevModel &m, const floa
                                                    int lane, int bar_id)
 {
     double e = 0.0;
-    constexpr int U = 4;                                     // columns per trip: all gathers of a trip in flight together
-    for (int i = warp; i < m.L - m.min_sep; i += nwarps) {
-        const float4 ci = cb4[i];
-        const int rb = tri_row(i, 0, m.L);
-        for (int j0 = i + m.min_sep + lane; j0 < m.L; j0 += 32 * U) {
+    // Work item = (row i, chunk q): the 32 columns j = i + min_sep + 32 q + lane.  A warp takes U rows of the same chunk
+    // per trip, so that U gathers are in flight per lane (a trip costs one L2 round trip whatever U is).
+    constexpr int U = 8;
+    const int nrow = m.L - m.min_sep;                        // rows with at least one column
+    for (int c0 = 0; c0 < nrow; c0 += 32) {
+        const int nr = nrow - c0;                            // rows that still have columns in this chunk
+        for (int i0 = warp; i0 < nr; i0 += nwarps * U) {
             float d2[U], f[U];
             float2 g[U];
+            int rj[U];
             float part = 0.0f;
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int j = min(j0 + 32 * u, m.L - 1);
-                const float4 cj = cb4[j];
+                const int i = i0 + u * nwarps;
+                const bool ok = i < nr;
+                const int ic = ok ? i : 0;
+                const int j = ic + m.min_sep + c0 + lane;
+                const float4 ci = cb4[ic];
+                const float4 cj = cb4[min(j, m.L - 1)];
                 const float dx = ci.x - cj.x, dy = ci.y - cj.y, dz = ci.z - cj.z;
-                d2[u] = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                d2[u] = (ok && j < m.L) ? fmaf(dx, dx, fmaf(dy, dy, dz * dz)) : m.far2;
+                rj[u] = tri_row(ic, 0, m.L) + j;
             }
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int j = j0 + 32 * u;
                 g[u] = make_float2(0.0f, 0.0f); f[u] = 0.0f;
-                if (j < m.L && d2[u] < m.far2) {
+                if (d2[u] < m.far2) {
                     int b;
                     bin_frac(d2[u], m.t0, m.inv_delta, m.tmax, m.thmax, b, f[u]);
-                    g[u] = __ldg(m.Epk + (size_t)(rb + j) * m.nb + b);
+                    g[u] = __ldg(m.Epk + (size_t)rj[u] * m.nb + b);
                 }
             }
 #pragma unroll
@@ -708,6 +725,7 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
 
     unsigned long long *full_bar = reinterpret_cast<unsigned long long *>(smem_raw);                 // [R]
     unsigned long long *empty_bar = full_bar + R;                                                     // [R]
+    const uint32_t full_bar_u32 = smem_u32(full_bar);
     float *ring = reinterpret_cast<float *>(smem_raw + sweep_header_bytes(R)) + (R > 0 ? kRingPadRows * m.row_stride : 0);
     const size_t chains_off = sweep_header_bytes(R) + ring_bytes(R, a.ring_rows, m.row_stride);
 
@@ -1127,9 +1145,13 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
                     while (seen_rel < need) {
                         ++seen_rel;
                         if (++seen_slot == R) { seen_slot = 0; seen_par ^= 1u; }
-                        mbar_wait(&full_bar[seen_slot], seen_par);
+                        mbar_wait_u32(full_bar_u32 + 8u * (uint32_t)seen_slot, seen_par);
                     }
-                    while (tb.c_ref < c_now) { ++tb.c_ref; if (++tb.slot_c == R) tb.slot_c = 0; }
+                    if (tb.c_ref < c_now) {                   // a pass advances by less than R columns
+                        tb.slot_c += c_now - tb.c_ref;
+                        if (tb.slot_c >= R) tb.slot_c -= R;
+                        tb.c_ref = c_now;
+                    }
                 }
                 const int r = gp ? warp : warp * gpw + grp;
                 const int gl_x = gp ? 32 : gl, glane_x = gp ? lane : glane;
@@ -1169,14 +1191,24 @@ __global__ void __launch_bounds__(kSweepMaxThreads, 1) sweep_kernel(DevModel m, 
 #pragma unroll
                             for (int q = 0; q < 3; ++q) rot_s[12 * r + 9 + q] = Rk.t[q];
                         }
-                        for (int jj = glane_x; jj < nJ; jj += gl_x) {
-                            const int j = split + jj;
-                            double x0, y0, z0, x, y, z;
-                            if (cb64) { x0 = X[3 * L + j]; y0 = Y[3 * L + j]; z0 = Z[3 * L + j]; }
-                            else cb_point(m, X, Y, Z, L, j, x0, y0, z0);
+                        // two columns per lane and trip, loads first (w + 1 = gl + 1 columns is the common case)
+                        for (int jj = glane_x; jj < nJ; jj += 2 * gl_x) {
+                            const int jj2 = jj + gl_x;
+                            const bool two = jj2 < nJ;
+                            const int j = split + jj, j2 = split + (two ? jj2 : jj);
+                            double x0, y0, z0, x, y, z, u0, v0, w0, u, v, w_;
+                            if (cb64) {
+                                x0 = X[3 * L + j]; y0 = Y[3 * L + j]; z0 = Z[3 * L + j];
+                                u0 = X[3 * L + j2]; v0 = Y[3 * L + j2]; w0 = Z[3 * L + j2];
+                            } else {
+                                cb_point(m, X, Y, Z, L, j, x0, y0, z0);
+                                cb_point(m, X, Y, Z, L, j2, u0, v0, w0);
+                            }
                             rot_apply(Rk, x0, y0, z0, x, y, z);
-                            AMH_ASSERT(jj < a.wpts && r < nspec && j < L, 7);
+                            rot_apply(Rk, u0, v0, w0, u, v, w_);
+                            AMH_ASSERT(jj < a.wpts && r < nspec && j < L && (!two || (jj2 < a.wpts && j2 < L)), 7);
                             cbn_r[jj] = make_float4((float)x, (float)y, (float)z, __int_as_float(col_term<RING>(tb, j)));
+                            if (two) cbn_r[jj2] = make_float4((float)u, (float)v, (float)w_, __int_as_float(col_term<RING>(tb, j2)));
                         }
                     }
                     __syncwarp();
