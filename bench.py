@@ -50,8 +50,8 @@ LANE_OPS_DISTANCE = 8           # of those, what a pair beyond the last bin cent
 # config 3 (fp64): arithmetic of one six-term pair counted from the formulas of R25, one op per add / multiply / fma, a root at 9
 # (reciprocal-root seed + Newton steps), atan2 at 45 (one division at 10, a degree-19 odd polynomial, octant fix-ups), an
 # interpolation at 8: distance 15 + 8; three dihedrals 3 x (9 + 12 + 9 + 9 + 1 + 45); two angles 2 x (6 + 6 + 6 + 9 + 45);
-# five more interpolations 40  = 462 -> 460.  (ncu counts 1.3x that in executed DADD + DMUL + DFMA per algorithmic pair:
-# profiles/r2_sass_pair_eval.md.)
+# five more interpolations 40  = 462 -> 460.  (ncu counts 414 executed DADD + DMUL + DFMA per algorithmic pair:
+# profiles/r2_ncu_per_config.md.)
 LANE_OPS_PER_PAIR_TR5 = 460
 FP32_LANES_PER_SM = 128
 FP64_LANES_PER_SM = 64
