@@ -250,6 +250,44 @@ amh_status amh_run_pt(amh_ctx *ctx, float *states, long long B, long long n_cycl
                       const amh_proposal *prop, unsigned long long seed, float *energy, float *best_energy,
                       unsigned long long *n_tried, unsigned long long *n_accepted, void *cuda_stream);
 
+/* amh_run_pt for callers that must not allocate device memory while they sample.
+ *
+ * amh_run_pt keeps one float per chain between a cycle's sweep kernel (which writes the cycle's best energy there) and
+ * the kernel that folds it into best_energy; it takes that room from the context's staging arena, which it grows with
+ * cudaMalloc (and cudaFree of the old arena) whenever a larger batch arrives.  Three kinds of caller cannot afford
+ * that inside their sampling loop:
+ *   - a sampler sharing the GPU with a framework whose caching allocator has already claimed nearly all of HBM
+ *     (PyTorch next to a resident model): a raw cudaMalloc then fails, or succeeds only after the framework is made
+ *     to hand blocks back;
+ *   - a service with a latency budget: cudaMalloc and cudaFree serialise against the whole device, so one call
+ *     stalls every other stream of the process, not just ours;
+ *   - code running under a "no allocation after start-up" rule (a fixed memory plan checked at start, or a region
+ *     in which the runtime refuses allocation calls outright).
+ * This entry point does the same work, enqueues the same kernels in the same order and leaves the same results, but
+ * its per-cycle scratch is a fixed array compiled into the library (file-scope __device__ storage,
+ * AMH_RUN_PT_STATIC_MAX_CHAINS floats = 256 KiB; every GPU on which the library is loaded carries it until the process
+ * exits).  It calls no cudaMalloc, no cudaFree and no library routine that allocates; the context itself is still
+ * built by amh_create, at start-up.
+ *
+ * Arguments, layouts and results: exactly amh_run_pt's (states, per_chain_T, energy, best_energy, n_tried, n_accepted
+ * are the caller's DEVICE buffers).  Differences:
+ *   - B > AMH_RUN_PT_STATIC_MAX_CHAINS returns AMH_ERR_UNSUPPORTED (amh_last_error names the limit) and enqueues
+ *     nothing.  Split a larger batch into several calls with chain_offset, one after the other.
+ *   - The device current at the call must be the one the context was created on (INVALID_ARG otherwise).
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress; it may also make the
+ *     runtime load the library's kernels).  Make that first call during start-up, before any stream capture begins
+ *     anywhere in the process.  Later calls on that device reuse the address.
+ *   - The array is shared by every call and every context of the process on that device, and keeps what the last
+ *     call left in it.  Nothing in it has to start at zero: each cycle's sweep kernel overwrites entries [0, B)
+ *     before they are read, so no call sees another's values - PROVIDED calls do not overlap on the GPU.  Two
+ *     calls in flight at once on different streams (or from different threads) race on it; order them on one
+ *     stream or with events. */
+#define AMH_RUN_PT_STATIC_MAX_CHAINS 65536
+amh_status amh_run_pt_static(amh_ctx *ctx, float *states, long long B, long long n_cycles, long long cycle_offset,
+                             long long chain_offset, const amh_schedule *sched, float *per_chain_T, int replicas,
+                             const amh_proposal *prop, unsigned long long seed, float *energy, float *best_energy,
+                             unsigned long long *n_tried, unsigned long long *n_accepted, void *cuda_stream);
+
 /* The same call on HOST buffers: states, temp->per_chain_T and every pointer in *out are host memory.
  * Copies in, runs, copies out and synchronises the stream; device staging buffers are owned by the
  * context and grow on demand. */

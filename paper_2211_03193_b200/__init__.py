@@ -17,14 +17,15 @@ import numpy as np
 
 from . import build as _build
 
-__all__ = ["AMH", "AMHError", "Options", "lib", "lib_path", "default_options", "philox4x32_10", "probe_l2_read", "probe_gather",
+__all__ = ["AMH", "AMHError", "RUN_PT_STATIC_MAX_CHAINS", "Options", "lib", "lib_path", "default_options", "philox4x32_10", "probe_l2_read", "probe_gather",
            "PROP_UNIFORM", "PROP_GRID", "PROP_GAUSSIAN", "EXPORTS"]
 
 PROP_UNIFORM, PROP_GRID, PROP_GAUSSIAN = 0, 1, 2
+RUN_PT_STATIC_MAX_CHAINS = 65536      # AMH_RUN_PT_STATIC_MAX_CHAINS of include/amh.h
 
 # every symbol include/amh.h declares
 EXPORTS = ["amh_default_options", "amh_default_launch_options", "amh_set_launch_options", "amh_create", "amh_destroy", "amh_energy", "amh_energy_local", "amh_coords",
-           "amh_create_tr5", "amh_pair_geometry", "amh_run", "amh_run_host", "amh_run_pt", "amh_exchange", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
+           "amh_create_tr5", "amh_pair_geometry", "amh_run", "amh_run_host", "amh_run_pt", "amh_run_pt_static", "amh_exchange", "amh_energy_host", "amh_launch_info", "amh_launch_shape", "amh_philox_test",
            "amh_probe_l2_read", "amh_probe_gather", "amh_launch_variant", "amh_check_status", "amh_last_error", "amh_version"]
 
 
@@ -127,6 +128,7 @@ def lib():
         L.amh_run_pt.argtypes = [C.c_void_p, C.c_void_p, C.c_longlong, C.c_longlong, C.c_longlong, C.c_longlong, C.c_void_p,
                                  C.c_void_p, C.c_int, C.c_void_p, C.c_ulonglong, C.c_void_p, C.c_void_p, C.c_void_p,
                                  C.c_void_p, C.c_void_p]
+        L.amh_run_pt_static.argtypes = L.amh_run_pt.argtypes
         L.amh_launch_info.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
         L.amh_launch_shape.argtypes = [C.c_void_p, C.c_longlong, C.c_int] + [C.POINTER(C.c_int)] * 4
         L.amh_probe_l2_read.argtypes = [C.c_longlong, C.c_int, C.POINTER(C.c_double), C.c_void_p]
@@ -401,6 +403,38 @@ class AMH:
                                 per_chain_T.data_ptr(), int(replicas), C.byref(pr), int(seed), energy.data_ptr(),
                                 best.data_ptr(), cnt[0:1].data_ptr(), cnt[1:2].data_ptr(), _stream_ptr(stream)))
         return dict(energy=energy, best_energy=best, n_swap_tried=cnt[0:1], n_swap_accepted=cnt[1:2])
+
+    def run_pt_static(self, states, n_cycles: int, per_chain_T, replicas: int, energy, best_energy=None, counters=None, *,
+                      n_global=1, n_local=2, window=8, global_first=True, prop_mode=PROP_UNIFORM, grid=0, sigma_start=0.0,
+                      sigma_end=0.0, ramp_sigma=0, seed=1, chain_offset=0, cycle_offset=0, stream=None):
+        """amh_run_pt_static: run_pt for callers that may not allocate device memory while they sample (a sampler
+        squeezed in beside a framework that owns nearly all of HBM, a latency-bound service that cannot take the
+        device-wide stall of cudaMalloc / cudaFree, code under a fixed memory plan).  The library's per-cycle scratch is
+        a fixed 256 KiB array inside the library instead of a staging arena, and this wrapper allocates nothing either:
+        EVERY buffer is the caller's, made once at start-up and reused -
+            states [B][n], per_chain_T [B], energy [B]   cuda float32, contiguous; updated / written in place
+            best_energy [B]                              cuda float32 or None
+            counters [2]                                 cuda int64 (swaps tried, swaps accepted; reset by the call) or None
+        B <= RUN_PT_STATIC_MAX_CHAINS, else AMHError (status UNSUPPORTED).  Results equal run_pt's.  Calls share the
+        library's array: do not let two of them run on the GPU at the same time (one stream, or events between them).
+        Make the first call on a device at start-up, before any stream capture in the process.  Returns None."""
+        torch = _torch()
+
+        def own(t, dtype, count, name):
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous() and t.numel() == count):
+                raise ValueError("%s must be a contiguous cuda %s tensor of %d elements (the caller owns every buffer)" % (name, dtype, count))
+            return t.data_ptr()
+        if not (isinstance(states, torch.Tensor) and states.numel() % self.n == 0):
+            raise ValueError("states must be a cuda float32 tensor [B][n]")
+        B = states.numel() // self.n
+        sc, _, pr = self._structs(n_global, n_local, window, global_first, 1.0, 1.0, 0, None, prop_mode, grid,
+                                  sigma_start, sigma_end, ramp_sigma)
+        cnt = own(counters, torch.int64, 2, "counters") if counters is not None else 0
+        _check(lib().amh_run_pt_static(self._h, own(states, torch.float32, B * self.n, "states"), B, int(n_cycles), int(cycle_offset),
+                                       int(chain_offset), C.byref(sc), own(per_chain_T, torch.float32, B, "per_chain_T"),
+                                       int(replicas), C.byref(pr), int(seed), own(energy, torch.float32, B, "energy"),
+                                       own(best_energy, torch.float32, B, "best_energy") if best_energy is not None else None,
+                                       cnt or None, (cnt + 8) if cnt else None, _stream_ptr(stream)))
 
     def run_host(self, states: np.ndarray, n_sweeps: int, *, n_global=1, n_local=10, window=8, global_first=True,
                  t_start=1.0, t_end=1.0, ramp_sweeps=0, per_chain_T=None, prop_mode=PROP_UNIFORM, grid=0,

@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "../../include/amh.h"
@@ -79,6 +80,37 @@ static amh_status check_launch_options(const amh_launch_options &o)
         return fail(AMH_ERR_INVALID_ARG, "launch options: lanes_per_step = %d not in {0, 4, 8, 16, 32}", o.lanes_per_step);
     if (o.spec_local < 0 || o.spec_local > amh::kMaxSpec)
         return fail(AMH_ERR_INVALID_ARG, "launch options: spec_local = %d outside [0, %d]", o.spec_local, amh::kMaxSpec);
+    return AMH_OK;
+}
+
+// ---- scratch of amh_run_pt_static (include/amh.h): the per-cycle best energies, one float per chain ---------------
+// Storage that is part of the library image instead of a cudaMalloc: each GPU that loads the library holds these
+// 256 KiB until the process exits.  Shared by every call on a device; see the header for what that means for callers.
+static __device__ __align__(256) float amh_pt_static_scratch[AMH_RUN_PT_STATIC_MAX_CHAINS];
+
+// In host code `amh_pt_static_scratch` is only a handle for the runtime, not something a kernel can dereference: the
+// address a kernel needs comes from cudaGetSymbolAddress, differs from device to device, and is looked up once per
+// device with that device current.  Host callers must never pass the bare name to a kernel.
+namespace {
+constexpr int kPtStaticMaxDevices = 64;
+std::mutex g_pt_static_mu;
+float *g_pt_static_addr[kPtStaticMaxDevices] = {};       // [device ordinal] -> device address, nullptr = not looked up yet
+}  // namespace
+
+static amh_status pt_static_scratch(int device, float **addr)
+{
+    if (device < 0 || device >= kPtStaticMaxDevices)
+        return fail(AMH_ERR_UNSUPPORTED, "amh_run_pt_static: device ordinal %d outside [0, %d)", device, kPtStaticMaxDevices);
+    std::lock_guard<std::mutex> lock(g_pt_static_mu);
+    if (!g_pt_static_addr[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, amh_pt_static_scratch);     // for the CURRENT device (checked by the caller)
+        if (e != cudaSuccess || !p)
+            return fail(AMH_ERR_CUDA, "amh_run_pt_static: cudaGetSymbolAddress on device %d: %s", device,
+                        e != cudaSuccess ? cudaGetErrorString(e) : "null address");
+        g_pt_static_addr[device] = static_cast<float *>(p);
+    }
+    *addr = g_pt_static_addr[device];
     return AMH_OK;
 }
 
@@ -856,6 +888,56 @@ amh_status amh_run_pt(amh_ctx *c, float *states, long long B, long long n_cycles
         amh_status stt = amh_run(c, states, B, cyc, y * cyc, chain_offset, sc, &tp, pr, seed, &o, cuda_stream);
         if (stt != AMH_OK) return stt;
         if (cycle_best && B > 0) {
+            amh::min_into_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(best_energy, cycle_best, B, y == cycle_offset);
+            AMH_CUDA(cudaGetLastError());
+        }
+        stt = amh_exchange(c, energy, per_chain_T, B, replicas, y, chain_offset, seed, n_tried, n_accepted, cuda_stream);
+        if (stt != AMH_OK) return stt;
+    }
+    return AMH_OK;
+}
+
+// amh_run_pt without the staging arena (include/amh.h says who needs this and why).  The loop below is amh_run_pt's,
+// kernel for kernel; the only difference is where the per-cycle best energies live: in amh_pt_static_scratch, reached
+// through the address pt_static_scratch() looked up for this device.  Nothing here may call cudaMalloc, cudaFree,
+// ensure_stage or anything else that allocates - tests/test_zz_no_alloc.py reads this body and checks that.
+amh_status amh_run_pt_static(amh_ctx *c, float *states, long long B, long long n_cycles, long long cycle_offset,
+                             long long chain_offset, const amh_schedule *sc, float *per_chain_T, int replicas,
+                             const amh_proposal *pr, unsigned long long seed, float *energy, float *best_energy,
+                             unsigned long long *n_tried, unsigned long long *n_accepted, void *cuda_stream)
+{
+    if (!c) return fail(AMH_ERR_INVALID_ARG, "amh_run_pt_static: ctx is NULL");
+    if (!sc || !per_chain_T || !energy) return fail(AMH_ERR_INVALID_ARG, "amh_run_pt_static: schedule / per_chain_T / energy is NULL");
+    if (n_cycles < 0 || cycle_offset < 0) return fail(AMH_ERR_INVALID_ARG, "amh_run_pt_static: n_cycles / cycle_offset < 0");
+    if (replicas < 2 || B % replicas || chain_offset % replicas)
+        return fail(AMH_ERR_INVALID_ARG, "amh_run_pt_static: B and chain_offset must be multiples of replicas >= 2");
+    if (B > (long long)AMH_RUN_PT_STATIC_MAX_CHAINS)
+        return fail(AMH_ERR_UNSUPPORTED, "amh_run_pt_static: B = %lld chains exceed the built-in scratch of AMH_RUN_PT_STATIC_MAX_CHAINS = %d "
+                    "(split the batch with chain_offset, or use amh_run_pt, which allocates)", B, (int)AMH_RUN_PT_STATIC_MAX_CHAINS);
+    int device = -1;
+    AMH_CUDA(cudaGetDevice(&device));
+    if (device != c->device)
+        return fail(AMH_ERR_INVALID_ARG, "amh_run_pt_static: the context lives on device %d, the current device is %d", c->device, device);
+    // first call on this device: the address look-up (and whatever the runtime loads with it) happens here
+    float *cycle_best = nullptr;
+    amh_status stt = pt_static_scratch(device, &cycle_best);
+    if (stt != AMH_OK) return stt;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (n_tried) AMH_CUDA(cudaMemsetAsync(n_tried, 0, sizeof(unsigned long long), st));
+    if (n_accepted) AMH_CUDA(cudaMemsetAsync(n_accepted, 0, sizeof(unsigned long long), st));
+    const long long cyc = (long long)sc->n_global + sc->n_local;
+    const bool want_best = best_energy && B > 0;
+    amh_temperature tp;
+    tp.t_start = tp.t_end = 1.0; tp.ramp_sweeps = 0; tp.per_chain_T = per_chain_T;
+    for (long long y = cycle_offset; y < cycle_offset + n_cycles; ++y) {
+        amh_outputs o;
+        std::memset(&o, 0, sizeof o);
+        // the sweep kernel stores the best energy of every row [0, B) at the end of the cycle: whatever an earlier
+        // call (of any batch size) left in the array is overwritten before min_into_kernel reads it - no clearing
+        o.energy = energy; o.best_energy = want_best ? cycle_best : nullptr;
+        stt = amh_run(c, states, B, cyc, y * cyc, chain_offset, sc, &tp, pr, seed, &o, cuda_stream);
+        if (stt != AMH_OK) return stt;
+        if (want_best) {
             amh::min_into_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(best_energy, cycle_best, B, y == cycle_offset);
             AMH_CUDA(cudaGetLastError());
         }
