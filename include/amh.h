@@ -158,7 +158,8 @@ amh_status amh_set_launch_options(amh_ctx *ctx, const amh_launch_options *opt);
  *   distogram   HOST or DEVICE float [L][L][n_bins] row-major, p_ij(b) >= 0 finite; only i < j is read.
  *               Copied: the caller may free it after the call.
  *   bin_edges   HOST float [n_bins + 1], increasing, evenly spaced to 1e-5 relative (else UNSUPPORTED)
- *   n_bins      >= 2
+ *   n_bins      >= 2; UNSUPPORTED when the packed pair table L (L - 1) / 2 x n_bins x 8 bytes (plus one row per residue)
+ *               reaches 2^31 bytes - the sweep kernel addresses it with 32-bit offsets (L = 600 allows 1,488 bins)
  *   opt         host, or NULL for the defaults
  * Synchronises the stream. */
 amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *distogram,

@@ -187,6 +187,16 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
             return fail(AMH_ERR_UNSUPPORTED, "amh_create: bins are not evenly spaced (bin %d: %g vs %g)", b, w, delta);
     }
 
+    {
+        // the local pair loop addresses the packed {E', slope} table with 32-bit byte offsets, row term + column term
+        // (LocalTab in amh_sweep.cuh): both terms and their sum must stay below 2^31
+        const unsigned long long rows = (unsigned long long)n_res * (n_res > 0 ? n_res - 1 : 0) / 2;
+        const unsigned long long reach = (rows + (unsigned long long)n_res + 1) * (unsigned long long)n_bins * 8ull;
+        if (reach >= (1ull << 31))
+            return fail(AMH_ERR_UNSUPPORTED, "amh_create: L = %d with n_bins = %d makes a pair table of %llu bytes; the sweep kernel "
+                        "addresses it with 32-bit offsets (limit 2^31 bytes)", n_res, n_bins, rows * (unsigned long long)n_bins * 8ull);
+    }
+
     amh_ctx *c = new (std::nothrow) amh_ctx;
     if (!c) return fail(AMH_ERR_OOM, "amh_create: host allocation failed");
     c->opt = o;

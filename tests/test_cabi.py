@@ -57,6 +57,11 @@ def test_default_options_and_argument_checks_without_a_device():
     assert lib.amh_probe_l2_read(16, 1, C.byref(v), None) == 1                                     # < 1 MiB
     assert lib.amh_create(C.byref(h), 2, 0, None, edges.ctypes.data, 64, None, None) == 1
     assert lib.amh_create(C.byref(h), 2, 0, p.ctypes.data, edges.ctypes.data, 1, None, None) == 1
+    # a pair table the sweep kernel's 32-bit offsets cannot span is refused before any device work (the distogram
+    # is not read that early, so a small stand-in serves): L = 600 holds 1,488 bins at most
+    wide = np.arange(1491, dtype=np.float32)                        # unit bins: evenly spaced exactly in fp32
+    assert lib.amh_create(C.byref(h), 600, 0, p.ctypes.data, wide.ctypes.data, 1490, None, None) == 2
+    assert b"32-bit offsets" in lib.amh_last_error()
     assert lib.amh_destroy(None) == 0
     assert lib.amh_energy(None, None, 0, None, None) == 1
 
