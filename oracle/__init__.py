@@ -344,6 +344,15 @@ def tr5_pair_geometry(s, geom: Geom | None = None):
     return tuple(out)
 
 
+def tr5_pair_geometry_atoms(N, CA, CB, i: int, j: int):
+    """amho_tr5_pair_geometry on atoms given directly (fp64 [L][3] each): d, omega, theta, phi of the ORDERED pair (i, j).
+    For pin P16, which places the atoms by hand."""
+    a = [np.ascontiguousarray(x, dtype=np.float64) for x in (N, CA, CB)]
+    v = [C.c_double() for _ in range(4)]
+    lib().amho_tr5_pair_geometry(_p(a[0]), _p(a[1]), _p(a[2]), C.c_int(i), C.c_int(j), *[C.byref(x) for x in v])
+    return tuple(x.value for x in v)
+
+
 class TR5Model:
     """Config 3's energy: tables E = -log(p + eps) in fp64 for the distance, omega, theta and phi maps."""
 

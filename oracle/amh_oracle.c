@@ -484,7 +484,9 @@ int amho_num_threads(void)
  *           + e_p[i][j](angle CA_i, CB_i, CB_j) + e_p[j][i](angle CA_j, CB_j, CB_i)                  12 bins over [0, pi], clamped
  *           every e = -log(p + eps) interpolated linearly between bin centres (circularly for the periodic ones)
  *   window  residue of variable k is floor(k/5); Eq. 3b and R12 unchanged
- * Parity unpinned: the parameterisation itself and the orientation conventions (the paper fixes neither).
+ * Parity unpinned: the CHOICE of the parameterisation and of the orientation conventions (the paper fixes neither).
+ * That amho_tr5_pair_geometry computes the conventions written above - which atoms, which order, which sign - is
+ * pinned by P16 (tests/test_oracle_tr5.py: two residues placed by hand, values derived from the coordinates).
  */
 typedef struct {
     int L, nb_d, nb_o, nb_t, nb_p;

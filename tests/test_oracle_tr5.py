@@ -108,6 +108,64 @@ def test_pair_geometry_symmetries_and_helix(orc):
             assert np.ptp(up) < 1e-9 and np.ptp(dn) < 1e-9
 
 
+def test_pair_geometry_on_hand_placed_atoms(orc):
+    # P16: WHICH atoms define omega, theta and phi, in which order and with which sign (R25; the definitions are the ones
+    # SURVEY.md 8(f) NEXT-2 writes out: omega = dihedral CA_i-CB_i-CB_j-CA_j, theta_ij = dihedral N_i-CA_i-CB_i-CB_j,
+    # phi_ij = angle CA_i-CB_i-CB_j).  Two residues placed by hand; every expected value is derived below from the
+    # coordinates alone.  A dihedral a-b-c-d is the rotation about b->c, right-handed, that carries the part of a - b
+    # normal to the axis onto the part of d - c normal to it.
+    r3 = math.sqrt(3.0)
+    CB = np.array([[0.0, 0.0, 0.0], [4.0, 0.0, 0.0]])                 # CB_0 -> CB_1 is +x, 4 A apart
+    CA = np.array([[1.0, 1.0, 0.0], [4.0, 1.0, r3]])
+    N = np.array([[2.0, 0.0, 1.0], [6.0, 1.0 + r3, r3 - 1.0]])
+    # d       = |CB_0 CB_1| = 4
+    # phi_01  = angle between CA_0 - CB_0 = (1, 1, 0) and +x: 45 deg
+    # phi_10  = angle between CA_1 - CB_1 = (0, 1, sqrt 3) and -x: 90 deg
+    # omega   : axis +x; CA_0 - CB_0 has normal part +y (azimuth 0), CA_1 - CB_1 = (0, 1, sqrt 3) sits at azimuth
+    #           +60 deg from y towards z, i.e. right-handed about +x: +60 deg, the same from either end
+    # theta_01: axis u = CA_0 -> CB_0 = -(1, 1, 0)/sqrt 2.  N_0 - CA_0 = (1, -1, 1) is normal to u; CB_1 - CB_0 = (4, 0, 0)
+    #           has normal part (2, -2, 0).  In the right-handed basis (e1 = z, e2 = u x z = (-1, 1, 0)/sqrt 2) the first
+    #           is (1, -sqrt 2)/sqrt 3, at -atan(sqrt 2) = -54.7356 deg, the second is -e2, at -90 deg:
+    #           theta_01 = -90 + 54.7356 = -atan(1/sqrt 2) = -35.2644 deg
+    # theta_10: axis u = CA_1 -> CB_1 = -(0, 1, sqrt 3)/2.  N_1 - CA_1 = (2, sqrt 3, -1) is normal to u; with
+    #           e1 = (0, sqrt 3, -1)/2 and e2 = u x e1 = +x it is 2 e1 + 2 e2, at +45 deg; CB_0 - CB_1 = -4 x = -4 e2, at
+    #           -90 deg: theta_10 = -90 - 45 = -135 deg
+    want01 = (4.0, 60.0, -math.degrees(math.atan(1.0 / math.sqrt(2.0))), 45.0)
+    want10 = (4.0, 60.0, -135.0, 90.0)
+    for (i, j), want in (((0, 1), want01), ((1, 0), want10)):
+        d, om, th, ph = orc.tr5_pair_geometry_atoms(N, CA, CB, i, j)
+        got = (d, math.degrees(om), math.degrees(th), math.degrees(ph))
+        assert np.allclose(got, want, rtol=0, atol=1e-9), ((i, j), got, want)
+    # the mirror image (z -> -z) flips both dihedrals and keeps the distance and the angle: the sign is a handedness
+    M = np.array([1.0, 1.0, -1.0])
+    d, om, th, ph = orc.tr5_pair_geometry_atoms(N * M, CA * M, CB * M, 0, 1)
+    assert np.allclose((d, math.degrees(om), math.degrees(th), math.degrees(ph)), (4.0, -60.0, -want01[2], 45.0), rtol=0, atol=1e-9)
+    # the pin has power: on these coordinates every near-miss reading gives another number (degrees, or A for d)
+    deg = lambda x: math.degrees(x)
+    miss = {
+        "theta as dihedral CA,N,CB,CB'": (deg(orc.dihedral(CA[0], N[0], CB[0], CB[1])), want01[2]),
+        "theta as dihedral N,CA,CB,CA'": (deg(orc.dihedral(N[0], CA[0], CB[0], CA[1])), want01[2]),
+        "theta_10 for theta_01": (want10[2], want01[2]),
+        "phi as angle N,CB,CB'": (deg(orc.angle(N[0], CB[0], CB[1])), want01[3]),
+        "phi as angle CA,CB,CA'": (deg(orc.angle(CA[0], CB[0], CA[1])), want01[3]),
+        "phi_10 for phi_01": (want10[3], want01[3]),
+        "omega as dihedral N,CB,CB',N'": (deg(orc.dihedral(N[0], CB[0], CB[1], N[1])), want01[1]),
+        "omega as dihedral CB,CA,CA',CB'": (deg(orc.dihedral(CB[0], CA[0], CA[1], CB[1])), want01[1]),
+        "omega for phi": (want01[1], want01[3]),
+        "d between the CAs": (float(np.linalg.norm(CA[0] - CA[1])), want01[0]),
+    }
+    for name, (other, right) in miss.items():
+        assert abs(other - right) > 0.5, name
+    # and the batch wrapper the synthetic maps are drawn from reads the same function in the same order:
+    # entry [i][j] is the ordered pair (i, j) - checked on a built chain against the per-pair call
+    s = gi.initial_states_tr5(1, 6, 8)[0]
+    Nn, CAn, Cn, CBn = orc.tr5_coords(s)
+    D, OM, TH, PH = orc.tr5_pair_geometry(s)
+    for i, j in ((0, 4), (4, 0), (2, 5)):
+        assert (D[i, j], OM[i, j], TH[i, j], PH[i, j]) == orc.tr5_pair_geometry_atoms(Nn, CAn, CBn, i, j)
+        assert abs(TH[i, j] - orc.dihedral(Nn[i], CAn[i], CBn[i], CBn[j])) < 1e-12 and abs(PH[i, j] - orc.angle(CAn[i], CBn[i], CBn[j])) < 1e-12
+
+
 def test_interpolation_periodic_and_clamped(orc):
     # P13: value at a bin centre = the table entry; circular: the seam is continuous and the midpoint between the last
     # and the first centre is their average; linear in between
