@@ -705,6 +705,9 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     if (c->param == AMH_PARAM_TR5) {
         // config 3: one CTA per chain, one proposal at a time (amh_tr5.cuh)
         const int threads = 128;
+        // 8 CTAs per SM against AMH_TR5_CTAS = 3 resident: chains differ in run time, and many short CTAs (1-2 rows each
+        // at B = 2,048) balance better than one resident wave striding over 4-5 rows (measured on config 3: 7,484 ms
+        // per step against 7,606 ms with n_sm * AMH_TR5_CTAS CTAs)
         const long long ctas = std::min<long long>(B, (long long)c->n_sm * 8);
         amh::tr5_sweep_kernel<<<(unsigned)ctas, threads, amh::tr5_smem_bytes(c->m.L, true), st>>>(c->tm, a);
         AMH_CUDA(cudaGetLastError());

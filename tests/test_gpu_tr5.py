@@ -50,6 +50,31 @@ def _angdiff(a, b):
     return np.minimum(d, np.abs(d - 2 * math.pi))
 
 
+def test_tr5_degenerate_geometry_scores_like_libm_atan2(amh, torch):
+    # cb_len = 0 puts every C-beta on its C-alpha: in omega = dihedral CA_i, CB_i, CB_j, CA_j the first bond vector
+    # is the zero vector, in theta = dihedral N_i, CA_i, CB_i, CB_j the axis is, in phi = angle CA_i, CB_i, CB_j one arm
+    # is: the device's branch-free atan2 is handed (+-0, +-0) exactly.  libm's atan2 (the oracle's) returns 0 or +-pi
+    # there, never +-pi/4 or +-3 pi/4 (which a zero vector sorted into the "diagonal" octant would give).  The oracle's
+    # own value is not compared: its projection form reaches the zero vector with other signs of zero, and its
+    # acos(0/0) is NaN for phi.
+    L = 7
+    flat = [np.full((L, L, nb), 1.0 / nb, np.float32) for nb in (37, 24, 24, 12)]
+    g = amh.AMH(flat[0], gi.bin_edges(37, 2.0, 20.0), amh.default_options(cb_len=0.0), orientation=flat[1:])
+    s = gi.initial_states_tr5(3, L, 5)
+    cb, at = g.coords(torch.from_numpy(s).cuda(), atoms=True)
+    at = at.cpu().numpy()
+    assert np.array_equal(at[:, :, 3], at[:, :, 1])                       # CB == CA, exactly
+    d, om, th, ph = [x.cpu().numpy() for x in g.pair_geometry(torch.from_numpy(s).cuda())]
+    off = ~np.eye(L, dtype=bool)
+    for name, a in (("omega", om), ("theta", th), ("phi", ph)):
+        v = np.abs(a[:, off])
+        assert np.all((v == 0.0) | (np.abs(v - math.pi) < 1e-15)), (name, np.unique(np.round(v, 6)))
+    assert np.all(d[:, off] > 1.0)                                        # the CAs themselves are apart
+    e = g.energy(torch.from_numpy(s).cuda()).cpu().numpy()
+    assert np.all(np.isfinite(e))
+    g.close()
+
+
 @pytest.mark.parametrize("L", [1, 2, 5, 33, 300])
 def test_tr5_coords_and_pair_geometry_parity(amh, orc, torch, tr5, L):
     ref, maps, edges, m, g = tr5(L)
