@@ -351,21 +351,39 @@ class Workload:
                  peak_source="derived: %d SMs x %d %s lanes x %.0f MHz (clocks.max.sm)" % (n_sm, lanes, "fp64" if fp64 else "fp32", sm_max_mhz),
                  hbm_gbs_measured=peaks.get("hbm_gbs"))
         if not fp64:
-            # a more conservative count: every pair needs its distance (8 lane-ops); only a near pair - and every in-window pair
-            # of a local proposal, where no far test is made - needs the other 20.  near fraction = the smaller of the start
-            # and the final states' (the states in between are at least as compact as the random start).
+            # `frac` charges a pair the arithmetic it needs: every pair its distance (8 lane-ops); only a near pair - and every
+            # in-window pair of a local proposal, where no far test is made - the other 20.  near fraction = the smaller of the
+            # start and the final states' (the states in between are at least as compact as the random start).  The all-pairs
+            # count of SURVEY.md 8(d) (every straddling pair at the full 28) is kept beside it: it charges the kernel work it
+            # skips exactly, and passes 1 where most pairs are far (config 4).
             f = min(self.near_fraction(self.s0_dev), self.near_fraction(self.states))
             gsum, lsum, allp = pair_counts(cfg.L, cfg.window, slots=cfg.slots)
             cyc = cfg.n_global + cfg.n_local
             full, rem = divmod(cfg.n_sweeps, cyc)
             n_g = full * cfg.n_global + min(rem, cfg.n_global)
             n_l = cfg.n_sweeps - n_g
-            ops = cfg.B * (n_l * lsum * LANE_OPS_PER_PAIR + (n_g * gsum + cfg.n_sweeps * allp) * (LANE_OPS_DISTANCE + f * (LANE_OPS_PER_PAIR - LANE_OPS_DISTANCE)))
-            r["frac_distance_weighted"] = ops / (ms_per_step * 1e-3) / 1e9 / peak
+            per_global_pair = LANE_OPS_DISTANCE + f * (LANE_OPS_PER_PAIR - LANE_OPS_DISTANCE)
+            ops_w = cfg.B * (n_l * lsum * LANE_OPS_PER_PAIR + (n_g * gsum + cfg.n_sweeps * allp) * per_global_pair)
+            per_s = 1.0 / (ms_per_step * 1e-3) / 1e9
+            r["achieved_all_pairs"], r["frac_all_pairs"] = r["achieved"], r["frac"]
+            r["frac_all_pairs_without_sweep_end_energy"] = cfg.B * (n_g * gsum + n_l * lsum) * LANE_OPS_PER_PAIR * per_s / peak
+            r["achieved"] = ops_w * per_s
+            r["frac"] = r["achieved"] / peak
+            r["frac_without_sweep_end_energy"] = cfg.B * (n_l * lsum * LANE_OPS_PER_PAIR + n_g * gsum * per_global_pair) * per_s / peak
             r["near_fraction"] = f
-            r["note"] = ("frac counts EVERY straddling pair at the %d lane-ops of a full evaluation (SURVEY.md 8(d)'s unit); the kernel skips pairs "
-                         "beyond the last bin centre exactly (their term is 0), so frac can exceed 1 where most pairs are far (config 4). "
-                         "frac_distance_weighted charges a far pair only its distance test (%d lane-ops)." % (LANE_OPS_PER_PAIR, LANE_OPS_DISTANCE))
+            r["note"] = ("achieved / frac charge a pair beyond the last bin centre only its distance test (%d lane-ops; its term is exactly 0 and "
+                         "the kernel skips it) and every other pair the %d lane-ops of a full evaluation; *_all_pairs charge EVERY straddling "
+                         "pair the full %d (SURVEY.md 8(d)'s unit) and can exceed 1 where most pairs are far (config 4); "
+                         "*_without_sweep_end_energy leave out the all-pairs energy of every sweep end (a9), which 8(d)'s pairs/proposal "
+                         "column does not contain." % (LANE_OPS_DISTANCE, LANE_OPS_PER_PAIR, LANE_OPS_PER_PAIR))
+            # a batch with fewer CTAs than SMs (config 0: 32 chains) cannot occupy the chip: the same figure against the SMs it can
+            ctas = -(-cfg.B // max(1, self.info["chains_per_cta"]))
+            if ctas < n_sm:
+                r["occupied_sms"] = ctas
+                r["frac_of_occupied_sms"] = r["frac"] * n_sm / ctas
+                r["frac_all_pairs_of_occupied_sms"] = r["frac_all_pairs"] * n_sm / ctas
+        if r["frac"] is not None and r["frac"] > 1.0:          # a fraction above 1 is a counting error, not a result
+            r["frac_rejected"], r["frac"] = r["frac"], None
         ipp = profiled_per_proposal(cfg.name, "thread_inst_per_proposal")
         if ipp is not None:
             r["executed_thread_inst_per_algorithmic_pair"] = ipp * cfg.proposals / pair_evals
