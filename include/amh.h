@@ -65,8 +65,16 @@ typedef struct {
                                                     guard_scale * G(L, window, extent) / T - G being the bound on the fp32
                                                     error of dE - is re-evaluated in fp64 (coordinates, root, -log(p + eps),
                                                     interpolation) before the decision is taken, so that every decision is
-                                                    the one fp64 arithmetic gives.  1 = default; 0 = off (fp32 decisions);
-                                                    a huge value sends every proposal through the fp64 path */
+                                                    the one fp64 arithmetic gives WHERE G BOUNDS THAT ERROR.  G is calibrated,
+                                                    not proven: about 4 x the largest error measured on distograms with a 5 %
+                                                    uniform floor (excess energies and bin-to-bin steps of the table up to 7.1),
+                                                    raised by (max(|E'|max, largest step) / 7.2)^2 for sharper tables - checked
+                                                    down to one-bin peaks without a floor at eps = 1e-8, where the error stays
+                                                    below a third of G (R24).  A smaller eps, or a chain that grows
+                                                    several-fold beyond 32 A within one sweep (the extent is sampled at sweep
+                                                    ends), is outside what was measured: raise guard_scale there.
+                                                    1 = default; 0 = off (fp32 decisions); a huge value sends every proposal
+                                                    through the fp64 path */
     int    min_sep;                              /* 3: pairs need j - i >= min_sep; >= 1 */
     int    pad_;
 } amh_options;

@@ -57,6 +57,7 @@ struct amh_ctx {
     float *Ebd = nullptr;        // the band j - i <= band_dmax of the same E', column-major, rows padded to row_stride floats (TMA source)
     int band_dmax = 0;
     float *P = nullptr;          // the probabilities themselves (fp64 path of the exact-decision guard)
+    float tab_emax = 0.0f, tab_step = 0.0f;   // max |E'| and max |E'[b+1] - E'[b]| of the table (table_kernel): scale the guard
     int param = AMH_PARAM_PHI_PSI;
     amh::Tr5Model tm;            // config 3 (AMH_PARAM_TR5): fp64 tables
     double *tE[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -291,8 +292,8 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
         AMH_CUDA_C(cudaMemsetAsync(c->Ebd, 0, bb, st));
     }
     AMH_CUDA_C(cudaMalloc(&c->P, sizeof(float) * n_rows * n_bins));
-    AMH_CUDA_C(cudaMalloc(&bad_dev, sizeof(int)));
-    AMH_CUDA_C(cudaMemsetAsync(bad_dev, 0, sizeof(int), st));
+    AMH_CUDA_C(cudaMalloc(&bad_dev, 3 * sizeof(int)));                // validity flag + the two table statistics
+    AMH_CUDA_C(cudaMemsetAsync(bad_dev, 0, 3 * sizeof(int), st));
     const float *src = distogram;
     if (!on_device) {
         AMH_CUDA_C(cudaMalloc(&p_dev, sizeof(float) * (size_t)count));
@@ -315,10 +316,13 @@ amh_status amh_create(amh_ctx **out, int n_res, amh_param param, const float *di
         cudaFree(vfar_dev);
         if (e_ != cudaSuccess) { cleanup(); return fail(AMH_ERR_CUDA, "amh_create: v_far: %s", cudaGetErrorString(e_)); }
     }
-    int bad = 0;
-    AMH_CUDA_C(cudaMemcpyAsync(&bad, bad_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
+    int bad3[3] = {0, 0, 0};
+    AMH_CUDA_C(cudaMemcpyAsync(bad3, bad_dev, sizeof bad3, cudaMemcpyDeviceToHost, st));
     AMH_CUDA_C(cudaStreamSynchronize(st));
+    const int bad = bad3[0];
     if (bad) { cleanup(); return fail(AMH_ERR_INVALID_ARG, "amh_create: the distogram holds a negative, NaN or infinite value"); }
+    std::memcpy(&c->tab_emax, &bad3[1], sizeof(float));
+    std::memcpy(&c->tab_step, &bad3[2], sizeof(float));
     cudaFree(bad_dev); bad_dev = nullptr;
     if (p_dev) { cudaFree(p_dev); p_dev = nullptr; }
     m.Epk = c->Epk; m.Elast = c->Elast; m.Ebd = c->Ebd; m.P = c->P;
@@ -687,8 +691,16 @@ amh_status amh_run(amh_ctx *c, float *states, long long B, long long n_sweeps, l
     a.seed = seed;
     {
         // exact-decision guard (R24): bound on |dE_fp32 - dE_fp64| at coordinates up to 32 A, scaled in the kernel by
-        // the chain's extent / 32 A.  Measured maxima with a safety factor of about 4.
-        const double gs = c->opt.guard_scale;
+        // the chain's extent / 32 A.  The constants are measured maxima with a safety factor of
+        // about 4 on tables whose excess energies and bin-to-bin steps stay below kGuardTableRef (BASELINE.json's
+        // distograms: 7.10 for both).  The fp32 error grows with both - the sums S_new, S_old grow with |E'|, the effect
+        // of a coordinate's rounding with the slope - so a sharper table raises the bound by the SQUARE of
+        // max(|E'|max, step max) / kGuardTableRef: measured on distograms without a uniform floor down to one-bin
+        // peaks (|E'| = step = 18.42, the most eps = 1e-8 allows: factor 6.5) the error grows 4-8.5 fold, and stays
+        // below a third of the scaled bound (profiles/r3_guard_sharp_tables.md).
+        constexpr double kGuardTableRef = 7.2;
+        const double sharp = std::max((double)c->tab_emax, (double)c->tab_step) / kGuardTableRef;
+        const double gs = c->opt.guard_scale * (sharp > 1.0 ? sharp * sharp : 1.0);
         const int w_eff = std::min(sc->window, std::max(c->m.L - 1, 0));
         a.guard_global = gs * 2e-3 * std::sqrt(std::max(c->m.L, 64) / 64.0);
         a.guard_local = gs * 1e-3 * std::sqrt((w_eff + 1) / 9.0);

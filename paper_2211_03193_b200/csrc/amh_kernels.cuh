@@ -13,9 +13,12 @@ __global__ void table_kernel(const float *__restrict__ p, float2 *__restrict__ E
                              float *__restrict__ Ebd, int band_rows, int min_sep, float *__restrict__ P, int row_stride, int L, int nb, double eps,
                              int *__restrict__ bad)
 {
+    // bad[0] = 1 if an entry is invalid; bad[1], bad[2] = bit patterns of max |E'| and max |E'[b+1] - E'[b]| over the
+    // pairs the energy reads (j - i >= min_sep): the exact-decision guard is scaled by them (amh_run, R24)
     const long long count = (long long)L * L * nb;
     const long long stride = (long long)gridDim.x * blockDim.x;
     int local_bad = 0;
+    float max_e = 0.0f, max_step = 0.0f;
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += stride) {
         const float v = p[q];
         if (!(v >= 0.0f) || isinf(v)) local_bad = 1;                 // every entry is validated, i >= j too
@@ -34,8 +37,16 @@ __global__ void table_kernel(const float *__restrict__ p, float2 *__restrict__ E
         if (q_ >= 0 && q_ < band_rows) Ebd[((long long)j * band_rows + q_) * row_stride + b] = e0;
         P[r * nb + b] = v;
         if (b == nb - 1) Elast[r] = (float)elast;
+        if (j - i >= min_sep) { max_e = fmaxf(max_e, fabsf(e0)); max_step = fmaxf(max_step, fabsf(de)); }
     }
     if (local_bad) atomicOr(bad, 1);
+    // non-negative floats order like their bit patterns
+    const unsigned be = __reduce_max_sync(0xffffffffu, __float_as_uint(max_e));
+    const unsigned bs = __reduce_max_sync(0xffffffffu, __float_as_uint(max_step));
+    if ((threadIdx.x & 31) == 0) {
+        if (be) atomicMax(reinterpret_cast<unsigned *>(bad) + 1, be);
+        if (bs) atomicMax(reinterpret_cast<unsigned *>(bad) + 2, bs);
+    }
 }
 
 // v_far = sum over the pairs j - i >= min_sep of -log(p[nb-1] + eps) in fp64 (one block, fixed order: deterministic)

@@ -147,7 +147,19 @@ def guard_bound(L, window, is_global, T=1.0):
     return 1e-3 * math.sqrt((min(window, L - 1) + 1) / 9.0)
 
 
-def _follow_check(m, s0, r, steps, **kw):
+def table_guard_factor(p, eps=1e-8, min_sep=3, ref=7.2):
+    """How amh_run scales the guard with the table (R24): the square of max(|E'|max, largest bin-to-bin step of E') / 7.2
+    where that exceeds 1; E' = E - E[last bin] as the kernel stores it (fp32), over the pairs j - i >= min_sep."""
+    L = p.shape[0]
+    iu = np.triu_indices(L, min_sep)
+    E = -np.log(p[iu].astype(np.float64) + eps)
+    Ep = (E - E[:, -1:]).astype(np.float32)
+    step = np.abs(np.diff(Ep, axis=1)) if Ep.size else np.zeros((0, 1), np.float32)
+    s = max(float(np.abs(Ep).max(initial=0.0)), float(step.max(initial=0.0))) / ref
+    return s * s if s > 1.0 else 1.0
+
+
+def _follow_check(m, s0, r, steps, bound_scale=1.0, **kw):
     """Follow-mode protocol: the oracle replays the GPU's decisions and checks its own.
     trace_acc bit 0 = accepted, bit 1 = decided by the fp64 path of the exact-decision guard (R24): there the
     traced dE must be the oracle's to fp64 rounding; everywhere else the fp32 dE must stay inside the guard's bound."""
@@ -170,7 +182,7 @@ def _follow_check(m, s0, r, steps, **kw):
     t = (kw.get("sweep_offset", 0) * n + np.arange(steps)) // n
     r_ = t % (ng + nl)
     is_g = (r_ < ng) if kw.get("global_first", True) else (r_ >= nl)
-    bound = np.where(is_g, guard_bound(L, 0, True), guard_bound(L, kw.get("window", 8), False))[None, :]
+    bound = bound_scale * np.where(is_g, guard_bound(L, 0, True), guard_bound(L, kw.get("window", 8), False))[None, :]
     ok = exact | (err < bound)
     assert ok.all(), "fp32 dE outside the guard's bound: %s (bound %s)" % (err[~ok], np.broadcast_to(bound, err.shape)[~ok])
     return dict(err=err, n_diff=int(diff.sum()), n_near=int(near.sum()), f=f, acc=acc, exact=exact, is_global=is_g)
@@ -636,6 +648,44 @@ def test_cold_end_of_config2_ramp(amh, orc, torch, synth, gpu_model):
         n_ex += int(chk["exact"].sum())
         assert 0.0 < chk["acc"].mean() < 0.5
     print("cfg2 cold end: %d of %d sampled steps decided by the fp64 path" % (n_ex, 8 * steps))
+
+
+@pytest.mark.parametrize("L", [64, 128])
+def test_sharp_distograms_keep_every_decision_exact(amh, orc, torch, L):
+    # R24 on tables far sharper than BASELINE.json's: no uniform floor (mix = 0: empty bins reach -log(1e-8) = 18.42) and
+    # peaks down to a single bin (sigma = 0.15 A against 0.3125 A bins).  The fp32 error of dE grows with the table's
+    # magnitude and steepness - 4 to 8.5 times the error on the benchmark tables - and passes the UNSCALED constants of the
+    # guard (column "of unscaled G" > 1); amh_run therefore scales them by table_guard_factor (6.5 here).  Checked at
+    # T = 1 and at T = 0.2 (where 1/T magnifies the error in the decision): every decision the oracle's, the fp32 dE
+    # of every step that was decided in fp32 inside the scaled bound with a margin of 2 (inside _follow_check: bound).
+    ref = gi.reference_torsions(L, 1000)
+    CB = orc.coords(ref)[3]
+    D = np.linalg.norm(CB[:, None] - CB[None], axis=-1)
+    edges = gi.bin_edges(64)
+    B, sweeps = 16, 44
+    s0 = gi.initial_states(B, 2 * L, seed=3)
+    kw = dict(n_global=1, n_local=10, window=8, seed=5)
+    steps = sweeps * 2 * L
+    assert table_guard_factor(gi.distogram_from_distances(D)) == 1.0          # the benchmark tables keep the constants as they were
+    for sigma in (1.0, 0.5, 0.3, 0.15):
+        p = gi.distogram_from_distances(D, sigma=sigma, mix=0.0)
+        fac = table_guard_factor(p)
+        assert 6.0 < fac < 7.0
+        m = orc.Model(p, edges)
+        g = amh.AMH(p, edges)
+        for T in (1.0, 0.2):
+            st = torch.from_numpy(s0.copy()).cuda()
+            r = g.run(st, sweeps, trace_steps=steps, t_start=T, t_end=T, **kw)
+            chk = _follow_check(m, s0, r, steps, bound_scale=0.5 * fac, t_start=T, t_end=T, **kw)
+            assert chk["n_diff"] == 0
+            assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+            err, ex, isg = chk["err"], chk["exact"], chk["is_global"]
+            eg, el = err[:, isg][~ex[:, isg]].max(), err[:, ~isg][~ex[:, ~isg]].max()
+            Gg, Gl = guard_bound(L, 0, True), guard_bound(L, 8, False)
+            print("sharp table L=%d sigma=%.2f mix=0 T=%.1f: guard factor %.2f; accepted %.3f, decided in fp64 %.5f; max fp32 |dE - oracle| global %.2e "
+                  "(%.2f of unscaled G, %.2f of scaled), local %.2e (%.2f of unscaled G, %.2f of scaled); decisions differing 0 of %d"
+                  % (L, sigma, T, fac, chk["acc"].mean(), ex.mean(), eg, eg / Gg, eg / (fac * Gg), el, el / Gl, el / (fac * Gl), err.size))
+        g.close()
 
 
 def test_error_codes(amh, torch, synth):
