@@ -688,6 +688,36 @@ def test_sharp_distograms_keep_every_decision_exact(amh, orc, torch, L):
         g.close()
 
 
+@pytest.mark.parametrize("stride", [0, 17])
+def test_hot_chains_stay_inside_the_guard_between_sweep_ends(amh, orc, torch, synth, gpu_model, stride):
+    # The guard's bound scales with the chain's extent (the fp32 rounding of large coordinates, R24), and the kernel samples
+    # the extent at sweep ends only.  At T = 10 a third of the proposals is accepted: a chain is rebuilt ~85 times per sweep
+    # and its extent moves between two samples - one chain starts as a 190 A helix and folds up.  Checked on both sweep
+    # orders (Alg. 1's and the strided one, which commits several moves at once): every decision the oracle's, the fp32 dE of
+    # every fp32-decided step inside the SMALLEST bound the kernel ever uses (_follow_check), few steps sent to the fp64 path.
+    # (A running upper bound of the extent across commits was tried in round 3: no decision changed, config 1 ran 2.2 %
+    # slower; include/amh.h states the sampling instead.)
+    L = 128
+    ref, p, edges, m = synth(L, 1001)
+    g = gpu_model(L, 1001)
+    B, sweeps = 12, 22
+    s0 = gi.initial_states(B, 2 * L, seed=8)
+    s0[0, 0::2] = np.float32(math.radians(-57.8)); s0[0, 1::2] = np.float32(math.radians(-47.0))    # a helix: 190 A long, folds up
+    kw = dict(n_global=1, n_local=10, window=8, seed=21, t_start=10.0, t_end=10.0)
+    if stride:
+        kw["local_stride"] = stride
+    steps = sweeps * 2 * L
+    st = torch.from_numpy(s0.copy()).cuda()
+    r = g.run(st, sweeps, trace_steps=steps, **kw)
+    chk = _follow_check(m, s0, r, steps, **kw)
+    assert chk["n_diff"] == 0
+    assert np.array_equal(st.cpu().numpy(), chk["f"]["states"])
+    assert chk["acc"].mean() > 0.25
+    assert chk["exact"].mean() < 0.01
+    print("hot chains (T = 10, stride %d): accepted %.3f, decided in fp64 %.5f, max fp32 |dE - oracle| %.2e"
+          % (stride, chk["acc"].mean(), chk["exact"].mean(), chk["err"][~chk["exact"]].max()))
+
+
 def test_error_codes(amh, torch, synth):
     ref, p, edges, m = synth(8, 1000)
     with pytest.raises(amh.AMHError) as e:
